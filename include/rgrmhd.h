@@ -1,0 +1,145 @@
+/* rgrmhd.h -- C-ABI of the B200-native resistive GRMHD IMEX-RK2 step.
+ *
+ * What it is: one full IMEX-SSP2(2,2,2) step (Eq. 35-37) of the resistive
+ * GRMHD conserved system (Eq. 22-29) on one uniform 3D Cartesian block with
+ * ghost zones and a fixed, externally supplied 3+1 metric (Eq. 1-5).  All
+ * arithmetic is FP64 and runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Field layout (every array argument): a padded structure-of-arrays field of
+ *     nxp * nyp * nzp doubles,   n?p = n? + 2*ng if n? > 1 else 1,   x fastest,
+ *     index(i,j,k) = (i+gx) + nxp*((j+gy) + nyp*(k+gz)),  g? = ng if n? > 1 else 0.
+ * Vector components are coordinate components: v^i, E^i, B^i, beta^i contravariant; S_i
+ * covariant; gamma_ij, K_ij covariant, stored xx,xy,xz,yy,yz,zz.
+ *
+ * Pointers: every field pointer may be a DEVICE pointer on params.device or a HOST pointer
+ * (pageable or pinned); the library classifies it with cudaPointerGetAttributes and issues
+ * the matching stream-ordered copy.  Pointer tables (the `const double* const x[14]`
+ * arguments) are HOST arrays of such pointers.  Host scalars/structs are written
+ * synchronously.
+ *
+ * Ownership: the handle owns all internal device memory.  Caller arrays are read (set_*) or
+ * written (get_*) by work enqueued during the call and are never retained.
+ *
+ * Ordering: all calls enqueue on the handle's stream (default: the legacy default stream;
+ * rgrmhd_set_stream changes it) and return without host synchronisation, except
+ * rgrmhd_max_speed and rgrmhd_get_stats (host scalars: they synchronise the stream) and
+ * copies from/to pageable host memory (synchronous by CUDA's rules).
+ *
+ * Errors: every function returns 0 on success or a negative rgrmhd_status.  No exceptions
+ * cross the ABI, there is no global state, and handles are not thread-safe.  A cell whose
+ * root solve does not converge is NOT an error: it keeps its last iterate (or the floor
+ * values) and is counted in rgrmhd_stats.
+ */
+#ifndef RGRMHD_H
+#define RGRMHD_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rgrmhd_s* rgrmhd_t;
+
+enum rgrmhd_status {
+  RGRMHD_OK        =  0,
+  RGRMHD_E_INVALID = -1, /* null pointer, ng != 3, n < 1, dx <= 0, Gamma <= 1, unknown enum     */
+  RGRMHD_E_STATE   = -2, /* step/get before set_metric + set_prims; set_sigma w/o ARRAY model  */
+  RGRMHD_E_CUDA    = -3, /* a CUDA call failed; rgrmhd_last_cuda_error() returns its string    */
+  RGRMHD_E_NOMEM   = -4  /* device allocation failed                                            */
+};
+
+/* boundary conditions ("Neumann": copy nearest interior cell; PAPER.md:359 periodic) */
+enum { RGRMHD_BC_PERIODIC = 0, RGRMHD_BC_OUTFLOW = 1 };
+
+/* conductivity models: uniform; per-cell array (BASELINE config 4); sigma0*(D/Dref)^exp
+ * (Eq. 52; D undensitised, exp a non-negative integer);
+ * sigma0*max(1 - D_atmo/D, 0)^2 (Eq. 61; sigma_dref = D_atmo). */
+enum { RGRMHD_SIGMA_UNIFORM = 0, RGRMHD_SIGMA_ARRAY = 1, RGRMHD_SIGMA_POWER_D = 2, RGRMHD_SIGMA_ATMO = 3 };
+
+/* how the conduction current in the charge flux (last row of Eq. 27) is evaluated at faces;
+ * the paper is silent (reading R3):
+ *   FACE_OHM     Ohm's law (Eq. 29) on the reconstructed left/right states, sigma_L/R = cell sigma
+ *   CELL_CURRENT (default) the cell-centred conduction current fixed by the implicit solve of the
+ *                same stage, J_c = (calE* - calE)/(a_ii dt alpha), reconstructed like a primitive
+ *   DIV_E        not evolved: q = div E after each stage -- NOT BUILT YET: create
+ *                returns RGRMHD_E_INVALID. */
+enum { RGRMHD_CHARGE_FACE_OHM = 0, RGRMHD_CHARGE_CELL_CURRENT = 1, RGRMHD_CHARGE_DIV_E = 2 };
+
+/* `scheme` argument of rgrmhd_step = reconstruction | time scheme */
+enum { RGRMHD_RECON_MINMOD = 0, RGRMHD_RECON_MC = 1, RGRMHD_RECON_WENO5 = 2, RGRMHD_RECON_MASK = 0xff };
+enum { RGRMHD_TIME_IMEX_SSP2_222 = 0 << 8, RGRMHD_TIME_MASK = 0xff00 };
+
+typedef struct {
+  int    n[3];        /* interior cells per direction; n = 1 marks an inactive direction          */
+  double dx[3];       /* cell sizes (> 0; ignored for inactive directions)                        */
+  int    ng;          /* ghost zones per side of an active direction; must be 3                   */
+  int    bc[3];       /* RGRMHD_BC_* per direction                                                */
+  double gamma_eos;   /* ideal-gas Gamma, p = (Gamma-1) rho eps (Eq. 49)            */
+  int    sigma_model; /* RGRMHD_SIGMA_*                                                           */
+  double sigma0, sigma_exp, sigma_dref;
+  double kappa;       /* divergence-cleaning damping (1)                            */
+  double rho_floor;   /* atmosphere density; 0 disables the floor                  */
+  double k_atmo;      /* polytropic K of the atmosphere, p = K rho^Gamma           */
+  double c2p_tol;     /* relative tolerance of the root solve; <= 0 selects 8*2^-52               */
+  int    c2p_max_iter;/* cap on residual evaluations per cell and solve; <= 0 selects 100         */
+  int    charge_mode; /* RGRMHD_CHARGE_*                                                          */
+  double weno_eps;    /* WENO5 regulariser; <= 0 selects 1e-26 (reading R5)             */
+  int    device;      /* CUDA device ordinal                                                      */
+} rgrmhd_params;
+
+typedef struct {
+  long long c2p_solves;     /* cell solves performed since create/reset                           */
+  long long c2p_evals;      /* residual evaluations summed over those solves                      */
+  long long c2p_failures;   /* solves that hit the cap or had no physical bracket                 */
+  long long floor_resets;   /* cells reset to the atmosphere                                      */
+  int       c2p_max_evals;  /* largest evaluation count of any single solve                       */
+  int       reserved;
+} rgrmhd_stats;
+
+/* Fill *p with the defaults documented above (kappa = 1, charge_mode = CELL_CURRENT, ...). */
+int rgrmhd_params_default(rgrmhd_params* p);
+
+/* Allocate a handle and all device state for the block. */
+int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p);
+int rgrmhd_destroy(rgrmhd_t h);
+
+/* Use `cuda_stream` (a cudaStream_t, e.g. torch's current stream) for all later work. */
+int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream);
+
+/* Fixed 3+1 metric: lapse, shift beta^i, gamma_ij, K_ij as padded
+ * fields INCLUDING ghost zones (the library never extrapolates a metric). */
+int rgrmhd_set_metric(rgrmhd_t h, const double* alpha, const double* const beta[3],
+                      const double* const gam[6], const double* const K[6]);
+
+/* Per-cell conductivity (SIGMA_ARRAY model only), padded field. */
+int rgrmhd_set_sigma(rgrmhd_t h, const double* sigma);
+
+/* Primitive state: rho,p,vx,vy,vz,Ex,Ey,Ez,Bx,By,Bz,psi,phi,q.  Also computes
+ * the conserved state (Eq. 22-24, 28).  Requires set_metric first. */
+int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]);
+
+/* One IMEX-SSP2(2,2,2) step of size dt (Eq. 35-37): implicit-E + recovery, ghost fill,
+ * reconstruction + HLLE + divergence + sources, stage combine; twice; final recovery. */
+int rgrmhd_step(rgrmhd_t h, double dt, int scheme);
+
+/* max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k
+ * (Eq. 30); dt = CFL / that.  Synchronises. */
+int rgrmhd_max_speed(rgrmhd_t h, double* host_out);
+
+/* Current primitives (ghost zones filled by the boundary rule) / conserved variables
+ * D,Sx,Sy,Sz,tau,calE(3),calB(3),Psi,Phi,calQ (interior valid; ghosts unspecified). */
+int rgrmhd_get_prims(rgrmhd_t h, double* const prims[14]);
+int rgrmhd_get_cons(rgrmhd_t h, double* const cons[14]);
+
+int rgrmhd_get_stats(rgrmhd_t h, rgrmhd_stats* host_out);   /* synchronises */
+int rgrmhd_reset_stats(rgrmhd_t h);
+
+/* Kernel launches enqueued by this handle since create (bench.py's "gpu_launches"). */
+int rgrmhd_launch_count(rgrmhd_t h, long long* host_out);
+
+const char* rgrmhd_strerror(int code);
+const char* rgrmhd_last_cuda_error(rgrmhd_t h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RGRMHD_H */

@@ -1,0 +1,233 @@
+"""CPU ORACLE loader (TEST INFRASTRUCTURE, NOT THE PRODUCT).
+
+Builds ``oracle/rgrmhd_oracle.cpp`` with ``g++ -O2 -ffp-contract=off`` and exposes it through
+ctypes.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package; ``paper_2510_18968_b200`` never does, and
+this package never imports the CUDA binding.
+
+Two builds of the same source: ``liboracle.so`` (single thread: the oracle by definition, and
+what ``cpu_baseline`` times) and ``liboracle_omp.so`` (``-fopenmp`` over independent cells, used
+only to make the large parity samples finish; results are thread-count independent).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Dict, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "rgrmhd_oracle.cpp")
+_LIBS: Dict[bool, C.CDLL] = {}
+
+NPRIM = NCONS = 14
+
+
+def build(force: bool = False) -> None:
+    """Compile both oracle variants in-tree (idempotent)."""
+    for omp in (False, True):
+        out = os.path.join(_HERE, "liboracle_omp.so" if omp else "liboracle.so")
+        if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
+            continue
+        cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-Wno-unknown-pragmas"]
+        if omp:
+            cmd.append("-fopenmp")
+        cmd += ["-o", out + ".tmp%d" % os.getpid(), _SRC]
+        subprocess.check_call(cmd)
+        os.replace(out + ".tmp%d" % os.getpid(), out)
+
+
+class Params(C.Structure):
+    _fields_ = [("n", C.c_int * 3), ("dx", C.c_double * 3), ("ng", C.c_int), ("bc", C.c_int * 3),
+                ("gamma_eos", C.c_double), ("sigma_model", C.c_int), ("sigma0", C.c_double),
+                ("sigma_exp", C.c_double), ("sigma_dref", C.c_double), ("kappa", C.c_double),
+                ("rho_floor", C.c_double), ("k_atmo", C.c_double), ("c2p_tol", C.c_double),
+                ("c2p_max_iter", C.c_int), ("charge_mode", C.c_int), ("weno_eps", C.c_double),
+                ("device", C.c_int)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("c2p_solves", C.c_longlong), ("c2p_evals", C.c_longlong), ("c2p_failures", C.c_longlong),
+                ("floor_resets", C.c_longlong), ("c2p_max_evals", C.c_int), ("reserved", C.c_int)]
+
+
+def lib(omp: bool = False) -> C.CDLL:
+    if omp not in _LIBS:
+        build()
+        L = C.CDLL(os.path.join(_HERE, "liboracle_omp.so" if omp else "liboracle.so"))
+        L.oracle_max_speed.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        for name in ("oracle_prim2cons_point", "oracle_c2p_point", "oracle_c2p_literal_point",
+                     "oracle_implicit_E_point", "oracle_state_flux_point", "oracle_recon_1d"):
+            getattr(L, name).restype = C.c_int
+        _LIBS[omp] = L
+    return _LIBS[omp]
+
+
+def _dp(a: Optional[np.ndarray]):
+    if a is None:
+        return None
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ptr_table(arrs: Sequence[np.ndarray]):
+    T = C.POINTER(C.c_double) * len(arrs)
+    return T(*[_dp(a) for a in arrs])
+
+
+def make_params(p: dict) -> Params:
+    q = Params()
+    q.n[:] = list(p["n"]); q.dx[:] = list(p["dx"]); q.ng = int(p.get("ng", 3)); q.bc[:] = list(p["bc"])
+    q.gamma_eos = p["gamma_eos"]; q.sigma_model = int(p.get("sigma_model", 0)); q.sigma0 = p.get("sigma0", 0.0)
+    q.sigma_exp = p.get("sigma_exp", 0.0); q.sigma_dref = p.get("sigma_dref", 1.0); q.kappa = p.get("kappa", 1.0)
+    q.rho_floor = p.get("rho_floor", 0.0); q.k_atmo = p.get("k_atmo", 0.0); q.c2p_tol = p.get("c2p_tol", 0.0)
+    q.c2p_max_iter = int(p.get("c2p_max_iter", 0)); q.charge_mode = int(p.get("charge_mode", 1))
+    q.weno_eps = p.get("weno_eps", 0.0); q.device = 0
+    return q
+
+
+class Oracle:
+    """Handle-level wrapper mirroring include/rgrmhd.h (host NumPy arrays)."""
+
+    def __init__(self, params: dict, omp: bool = False):
+        self.L = lib(omp)
+        self.par = make_params(params)
+        self.h = C.c_void_p()
+        rc = self.L.oracle_create(C.byref(self.h), C.byref(self.par))
+        if rc != 0:
+            raise ValueError("oracle_create failed: %d" % rc)
+        n = params["n"]
+        self.shape = tuple(int(m + 6) if m > 1 else 1 for m in (n[2], n[1], n[0]))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.L.oracle_destroy(self.h)
+            self.h = None
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise RuntimeError("%s failed: %d" % (what, rc))
+
+    def set_metric(self, metric: np.ndarray):
+        m = np.ascontiguousarray(metric, dtype=np.float64)
+        assert m.shape == (16,) + self.shape, (m.shape, self.shape)
+        self._check(self.L.oracle_set_metric(self.h, _dp(m[0]), _ptr_table([m[1], m[2], m[3]]),
+                                             _ptr_table([m[4 + i] for i in range(6)]),
+                                             _ptr_table([m[10 + i] for i in range(6)])), "set_metric")
+
+    def set_sigma(self, sigma: np.ndarray):
+        s = np.ascontiguousarray(sigma, dtype=np.float64)
+        assert s.shape == self.shape
+        self._check(self.L.oracle_set_sigma(self.h, _dp(s)), "set_sigma")
+
+    def set_prims(self, prims: np.ndarray):
+        p = np.ascontiguousarray(prims, dtype=np.float64)
+        assert p.shape == (14,) + self.shape
+        self._check(self.L.oracle_set_prims(self.h, _ptr_table([p[i] for i in range(14)])), "set_prims")
+
+    def step(self, dt: float, scheme: int):
+        self._check(self.L.oracle_step(self.h, C.c_double(dt), int(scheme)), "step")
+
+    def max_speed(self) -> float:
+        out = C.c_double()
+        self._check(self.L.oracle_max_speed(self.h, C.byref(out)), "max_speed")
+        return out.value
+
+    def get_prims(self) -> np.ndarray:
+        p = np.empty((14,) + self.shape)
+        self._check(self.L.oracle_get_prims(self.h, _ptr_table([p[i] for i in range(14)])), "get_prims")
+        return p
+
+    def get_cons(self) -> np.ndarray:
+        u = np.empty((14,) + self.shape)
+        self._check(self.L.oracle_get_cons(self.h, _ptr_table([u[i] for i in range(14)])), "get_cons")
+        return u
+
+    def rhs(self, scheme: int) -> np.ndarray:
+        f = np.empty((14,) + self.shape)
+        self._check(self.L.oracle_rhs(self.h, int(scheme), _ptr_table([f[i] for i in range(14)])), "rhs")
+        return f
+
+    def ghost_fill(self, field: np.ndarray) -> np.ndarray:
+        f = np.ascontiguousarray(field, dtype=np.float64).copy()
+        self._check(self.L.oracle_ghost_fill(self.h, _dp(f)), "ghost_fill")
+        return f
+
+    def stats(self) -> dict:
+        s = Stats()
+        self._check(self.L.oracle_get_stats(self.h, C.byref(s)), "get_stats")
+        return {k: getattr(s, k) for k, _ in Stats._fields_ if k != "reserved"}
+
+    def reset_stats(self):
+        self.L.oracle_reset_stats(self.h)
+
+
+def from_workload(w, fields: Optional[dict] = None, omp: bool = False, n=None, bc=None, **over) -> Oracle:
+    """Create an oracle handle for workload `w` (or a sub-block of it) and load its fields."""
+    par = w.params(n=n, bc=bc)
+    par.update(over)
+    o = Oracle(par, omp=omp)
+    f = fields if fields is not None else w.fields()
+    o.set_metric(f["metric"])
+    if f["sigma"] is not None and par["sigma_model"] == 1:
+        o.set_sigma(f["sigma"])
+    o.set_prims(f["prims"])
+    return o
+
+
+# ---- point-wise wrappers (used by the pins) -------------------------------------------------------
+_G_FLAT = np.array([1.0, 0, 0, 1.0, 0, 1.0])
+
+
+def _a(x, n=None):
+    a = np.ascontiguousarray(x, dtype=np.float64)
+    if n is not None:
+        assert a.shape == (n,)
+    return a
+
+
+def prim2cons_point(P, gamma_eos, alpha=1.0, beta=None, g6=None):
+    U = np.empty(14)
+    lib().oracle_prim2cons_point(C.c_double(gamma_eos), C.c_double(alpha), _dp(_a(beta, 3)) if beta is not None else None,
+                                 _dp(_a(_G_FLAT if g6 is None else g6, 6)), _dp(_a(P, 14)), _dp(U))
+    return U
+
+
+def c2p_point(U, guess, gamma_eos, adt=0.0, sigma=0.0, alpha=1.0, g6=None, tol=0.0, maxit=0, literal=False):
+    """Returns (prims, evals, failed)."""
+    P = _a(guess, 14).copy()
+    fn = lib().oracle_c2p_literal_point if literal else lib().oracle_c2p_point
+    if literal and tol <= 0:
+        tol = 1e-13
+    if literal and maxit <= 0:
+        maxit = 100
+    r = fn(C.c_double(gamma_eos), C.c_double(alpha), _dp(_a(_G_FLAT if g6 is None else g6, 6)), _dp(_a(U, 14)),
+           C.c_double(adt), C.c_double(sigma), C.c_double(tol), C.c_int(maxit), _dp(P))
+    return P, abs(r), r < 0
+
+
+def implicit_E_point(v, s, Estar, B, alpha=1.0, g6=None, newton=False, E0=None, iters=1):
+    E = np.empty(3)
+    E0 = _a(np.zeros(3) if E0 is None else E0, 3)
+    lib().oracle_implicit_E_point(C.c_double(alpha), _dp(_a(_G_FLAT if g6 is None else g6, 6)), _dp(_a(v, 3)),
+                                  C.c_double(s), _dp(_a(Estar, 3)), _dp(_a(B, 3)), C.c_int(1 if newton else 0),
+                                  _dp(E0), C.c_int(iters), _dp(E))
+    return E
+
+
+def state_flux_point(P, k, gamma_eos, alpha=1.0, beta=None, g6=None, charge_mode=1, sigma=0.0, jck=0.0):
+    U = np.empty(14); F = np.empty(14)
+    lib().oracle_state_flux_point(C.c_double(gamma_eos), C.c_double(alpha), _dp(_a(beta, 3)) if beta is not None else None,
+                                  _dp(_a(_G_FLAT if g6 is None else g6, 6)), C.c_int(k), _dp(_a(P, 14)),
+                                  C.c_int(charge_mode), C.c_double(sigma), C.c_double(jck), _dp(U), _dp(F))
+    return U, F
+
+
+def recon_1d(u, scheme, eps_w=0.0):
+    u = _a(u)
+    lo = np.full_like(u, np.nan); hi = np.full_like(u, np.nan)
+    lib().oracle_recon_1d(C.c_int(scheme), C.c_double(eps_w), C.c_int(u.size), _dp(u), _dp(lo), _dp(hi))
+    return lo, hi
