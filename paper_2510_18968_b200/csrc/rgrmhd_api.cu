@@ -1,0 +1,360 @@
+// rgrmhd_api.cu -- host driver and C-ABI (include/rgrmhd.h) of the B200-native resistive GRMHD step.
+// Stage sequencing of IMEX-SSP2(2,2,2) (Eq. 35-37), device buffers, stream.
+// There is no CPU fallback: every step of the path runs in the kernels of this library.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/rgrmhd.h"
+#include "rgrmhd_common.cuh"
+
+namespace rg {
+cudaError_t launch_c2p(const GridView& G, double* const Ust[NCONS], double* const Xout[3], double adt,
+                       bool write_back_floor, StatsDev* stats, cudaStream_t st);
+cudaError_t launch_prim2cons(const GridView& G, cudaStream_t st);
+cudaError_t launch_rhs_simple(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
+cudaError_t launch_rhs_tiled(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
+bool rhs_tiled_supported(const GridView& G);
+cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, cudaStream_t st);
+cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, cudaStream_t st);
+}  // namespace rg
+
+struct rgrmhd_s {
+  rgrmhd_params par;
+  rg::GridView G;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  double* slab = nullptr;            // all fields, one allocation
+  long long field_stride = 0;        // doubles between consecutive fields (ntot rounded up to 32)
+  rg::StatsDev* stats_dev = nullptr;
+  unsigned long long* maxspeed_dev = nullptr;
+  long long solves = 0;              // host-side count of cell solves enqueued
+  long long launches = 0;
+  bool have_metric = false, have_prims = false, have_sigma = false;
+  int rhs_variant = 0;               // 0 = tiled (default), 1 = simple
+  std::string last_error;
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; }
+    if (prev != dev) ok = (cudaSetDevice(dev) == cudaSuccess);
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int fail_cuda(rgrmhd_t h, cudaError_t e, const char* what) {
+  if (h) h->last_error = std::string(what) + ": " + cudaGetErrorString(e);
+  return RGRMHD_E_CUDA;
+}
+
+#define RG_CUDA(h, call)                                            \
+  do {                                                              \
+    cudaError_t e__ = (call);                                       \
+    if (e__ != cudaSuccess) return fail_cuda((h), e__, #call);      \
+  } while (0)
+
+}  // namespace
+
+extern "C" {
+
+int rgrmhd_params_default(rgrmhd_params* p) {
+  if (!p) return RGRMHD_E_INVALID;
+  std::memset(p, 0, sizeof(*p));
+  for (int d = 0; d < 3; ++d) { p->n[d] = 1; p->dx[d] = 1.0; p->bc[d] = RGRMHD_BC_OUTFLOW; }
+  p->ng = 3;
+  p->gamma_eos = 4.0 / 3.0;
+  p->sigma_model = RGRMHD_SIGMA_UNIFORM;
+  p->sigma0 = 0.0; p->sigma_exp = 0.0; p->sigma_dref = 1.0;
+  p->kappa = 1.0;
+  p->rho_floor = 0.0; p->k_atmo = 0.0;
+  p->c2p_tol = 0.0; p->c2p_max_iter = 0;
+  p->charge_mode = RGRMHD_CHARGE_CELL_CURRENT;
+  p->weno_eps = 0.0;
+  p->device = 0;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
+  if (!out || !p) return RGRMHD_E_INVALID;
+  *out = nullptr;
+  if (p->ng != 3 || !(p->gamma_eos > 1.0)) return RGRMHD_E_INVALID;
+  for (int d = 0; d < 3; ++d) {
+    if (p->n[d] < 1) return RGRMHD_E_INVALID;
+    if (p->n[d] > 1 && !(p->dx[d] > 0.0)) return RGRMHD_E_INVALID;
+    if (p->n[d] > 1 && p->n[d] < 3) return RGRMHD_E_INVALID;   // periodic wrap of 3 ghosts needs >= 3 cells
+    if (p->bc[d] != RGRMHD_BC_PERIODIC && p->bc[d] != RGRMHD_BC_OUTFLOW) return RGRMHD_E_INVALID;
+  }
+  if (p->sigma_model < RGRMHD_SIGMA_UNIFORM || p->sigma_model > RGRMHD_SIGMA_ATMO) return RGRMHD_E_INVALID;
+  if (p->charge_mode != RGRMHD_CHARGE_FACE_OHM && p->charge_mode != RGRMHD_CHARGE_CELL_CURRENT)
+    return RGRMHD_E_INVALID;                                     // DIV_E: not built
+  if (p->sigma_model == RGRMHD_SIGMA_POWER_D &&
+      (p->sigma_exp < 0.0 || std::fabs(p->sigma_exp - std::lround(p->sigma_exp)) > 0.0 || !(p->sigma_dref > 0.0)))
+    return RGRMHD_E_INVALID;
+  if (p->weno_eps > 0.0 && p->weno_eps < 1e-60) return RGRMHD_E_INVALID;   // product-form weights would underflow
+  if (p->rho_floor < 0.0 || !(p->kappa == p->kappa)) return RGRMHD_E_INVALID;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || p->device < 0 || p->device >= ndev) {
+    cudaGetLastError();
+    return RGRMHD_E_CUDA;
+  }
+  rgrmhd_s* h = new (std::nothrow) rgrmhd_s();
+  if (!h) return RGRMHD_E_NOMEM;
+  h->par = *p;
+  h->device = p->device;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) { delete h; return RGRMHD_E_CUDA; }
+
+  rg::GridView& G = h->G;
+  std::memset(&G, 0, sizeof(G));
+  G.ntot = 1;
+  for (int d = 0; d < 3; ++d) {
+    G.n[d] = p->n[d];
+    G.g[d] = p->n[d] > 1 ? 3 : 0;
+    G.np[d] = p->n[d] + 2 * G.g[d];
+    G.bc[d] = p->bc[d];
+    G.dx[d] = p->dx[d];
+    G.inv_dx[d] = p->n[d] > 1 ? 1.0 / p->dx[d] : 0.0;
+    G.inv_12dx[d] = p->n[d] > 1 ? 1.0 / (12.0 * p->dx[d]) : 0.0;
+    G.ntot *= G.np[d];
+  }
+  G.stride[0] = 1; G.stride[1] = G.np[0]; G.stride[2] = (long long)G.np[0] * G.np[1];
+  G.Gamma = p->gamma_eos;
+  G.sigma_model = p->sigma_model; G.sigma0 = p->sigma0; G.sigma_dref = p->sigma_dref;
+  G.sigma_exp = (int)std::lround(p->sigma_exp);
+  G.kappa = p->kappa;
+  G.rho_floor = p->rho_floor;
+  G.p_atmo = p->rho_floor > 0.0 ? p->k_atmo * std::pow(p->rho_floor, p->gamma_eos) : 0.0;   // p = K rho^Gamma
+  G.tol = p->c2p_tol > 0.0 ? p->c2p_tol : 8.0 * std::ldexp(1.0, -52);
+  G.maxit = p->c2p_max_iter > 0 ? p->c2p_max_iter : 100;
+  G.charge_mode = p->charge_mode;
+  G.weno_eps = p->weno_eps > 0.0 ? p->weno_eps : 1e-26;
+
+  const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3;
+  h->field_stride = (G.ntot + 31) / 32 * 32;
+  const size_t bytes = (size_t)nfields * (size_t)h->field_stride * sizeof(double);
+  cudaError_t e = cudaMalloc((void**)&h->slab, bytes);
+  if (e != cudaSuccess) { cudaGetLastError(); delete h; return RGRMHD_E_NOMEM; }
+  e = cudaMalloc((void**)&h->stats_dev, sizeof(rg::StatsDev) + sizeof(unsigned long long));
+  if (e != cudaSuccess) { cudaGetLastError(); cudaFree(h->slab); delete h; return RGRMHD_E_NOMEM; }
+  h->maxspeed_dev = (unsigned long long*)(h->stats_dev + 1);
+  cudaMemset(h->slab, 0, bytes);
+  cudaMemset(h->stats_dev, 0, sizeof(rg::StatsDev) + sizeof(unsigned long long));
+  double* q = h->slab;
+  auto next = [&]() { double* r = q; q += h->field_stride; return r; };
+  for (int v = 0; v < rg::NMET; ++v) G.met[v] = next();
+  { double* s = next(); G.sigma = (p->sigma_model == RGRMHD_SIGMA_ARRAY) ? s : nullptr; }
+  for (int v = 0; v < rg::NPRIM; ++v) G.P[v] = next();
+  for (int v = 0; v < 3; ++v) G.jc[v] = next();
+  for (int v = 0; v < rg::NCONS; ++v) G.Un[v] = next();
+  for (int v = 0; v < rg::NCONS; ++v) G.Us[v] = next();
+  for (int v = 0; v < 3; ++v) G.X1[v] = next();
+  e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) { cudaFree(h->slab); cudaFree(h->stats_dev); delete h; return RGRMHD_E_CUDA; }
+  *out = h;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_destroy(rgrmhd_t h) {
+  if (!h) return RGRMHD_E_INVALID;
+  {
+    DeviceGuard guard(h->device);
+    cudaStreamSynchronize(h->stream);
+    cudaFree(h->slab);
+    cudaFree(h->stats_dev);
+  }
+  delete h;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream) {
+  if (!h) return RGRMHD_E_INVALID;
+  h->stream = (cudaStream_t)cuda_stream;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant) {
+  if (!h || variant < 0 || variant > 1) return RGRMHD_E_INVALID;
+  h->rhs_variant = variant;
+  return RGRMHD_OK;
+}
+
+static int copy_in(rgrmhd_t h, const double* dst_dev, const double* src) {
+  RG_CUDA(h, cudaMemcpyAsync((void*)dst_dev, src, (size_t)h->G.ntot * sizeof(double), cudaMemcpyDefault, h->stream));
+  return RGRMHD_OK;
+}
+static int copy_out(rgrmhd_t h, double* dst, const double* src_dev) {
+  RG_CUDA(h, cudaMemcpyAsync(dst, src_dev, (size_t)h->G.ntot * sizeof(double), cudaMemcpyDefault, h->stream));
+  return RGRMHD_OK;
+}
+
+int rgrmhd_set_metric(rgrmhd_t h, const double* alpha, const double* const beta[3], const double* const gam[6],
+                      const double* const K[6]) {
+  if (!h || !alpha || !beta || !gam || !K) return RGRMHD_E_INVALID;
+  for (int i = 0; i < 3; ++i) if (!beta[i]) return RGRMHD_E_INVALID;
+  for (int i = 0; i < 6; ++i) if (!gam[i] || !K[i]) return RGRMHD_E_INVALID;
+  DeviceGuard guard(h->device);
+  int rc;
+  if ((rc = copy_in(h, h->G.met[rg::MALP], alpha))) return rc;
+  for (int i = 0; i < 3; ++i) if ((rc = copy_in(h, h->G.met[rg::MBX + i], beta[i]))) return rc;
+  for (int i = 0; i < 6; ++i) {
+    if ((rc = copy_in(h, h->G.met[rg::MGXX + i], gam[i]))) return rc;
+    if ((rc = copy_in(h, h->G.met[rg::MKXX + i], K[i]))) return rc;
+  }
+  h->have_metric = true;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_set_sigma(rgrmhd_t h, const double* sigma) {
+  if (!h || !sigma) return RGRMHD_E_INVALID;
+  if (h->par.sigma_model != RGRMHD_SIGMA_ARRAY) return RGRMHD_E_STATE;
+  DeviceGuard guard(h->device);
+  int rc;
+  if ((rc = copy_in(h, h->G.sigma, sigma))) return rc;
+  h->have_sigma = true;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]) {
+  if (!h || !prims) return RGRMHD_E_INVALID;
+  for (int v = 0; v < rg::NPRIM; ++v) if (!prims[v]) return RGRMHD_E_INVALID;
+  if (!h->have_metric) return RGRMHD_E_STATE;
+  DeviceGuard guard(h->device);
+  int rc;
+  for (int v = 0; v < rg::NPRIM; ++v) if ((rc = copy_in(h, h->G.P[v], prims[v]))) return rc;
+  for (int q = 0; q < 3; ++q)
+    RG_CUDA(h, cudaMemsetAsync(h->G.jc[q], 0, (size_t)h->G.ntot * sizeof(double), h->stream));
+  RG_CUDA(h, rg::launch_prim2cons(h->G, h->stream));
+  ++h->launches;
+  h->have_prims = true;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
+  if (!h || !(dt > 0.0)) return RGRMHD_E_INVALID;
+  const int recon = scheme & RGRMHD_RECON_MASK;
+  if (recon > RGRMHD_RECON_WENO5 || (scheme & ~RGRMHD_RECON_MASK) != RGRMHD_TIME_IMEX_SSP2_222) return RGRMHD_E_INVALID;
+  if (!h->have_metric || !h->have_prims || (h->par.sigma_model == RGRMHD_SIGMA_ARRAY && !h->have_sigma))
+    return RGRMHD_E_STATE;
+  DeviceGuard guard(h->device);
+  const rg::GridView& G = h->G;
+  cudaStream_t st = h->stream;
+  const double gam = 1.0 - 1.0 / std::sqrt(2.0);
+  const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
+  double* ghost_fields[rg::NPRIM + 3];
+  for (int v = 0; v < rg::NPRIM; ++v) ghost_fields[v] = G.P[v];
+  for (int q = 0; q < 3; ++q) ghost_fields[rg::NPRIM + q] = G.jc[q];
+  const int nghost_fields = rg::NPRIM + (G.charge_mode == rg::CHARGE_CELL_CURRENT ? 3 : 0);
+  const bool any_active = G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1;
+  const bool tiled = h->rhs_variant == 0 && rg::rhs_tiled_supported(G);
+  auto rhs = [&](int stage) {
+    return tiled ? rg::launch_rhs_tiled(G, dt, stage, recon, st) : rg::launch_rhs_simple(G, dt, stage, recon, st);
+  };
+  // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n
+  RG_CUDA(h, rg::launch_c2p(G, G.Un, G.X1, gam * dt, false, h->stats_dev, st));
+  RG_CUDA(h, rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st));
+  RG_CUDA(h, rhs(1));                                         // -> U*2 (Eq. 36)
+  // stage 2 (Eq. 36)
+  RG_CUDA(h, rg::launch_c2p(G, G.Us, nullptr, gam * dt, false, h->stats_dev, st));
+  RG_CUDA(h, rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st));
+  RG_CUDA(h, rhs(2));                                         // -> U^{n+1} (Eq. 37)
+  // recovery of the new state at fixed calE (reading R12)
+  RG_CUDA(h, rg::launch_c2p(G, G.Un, nullptr, 0.0, true, h->stats_dev, st));
+  h->solves += 3 * nint;
+  h->launches += 5 + (any_active ? 2 : 0);
+  return RGRMHD_OK;
+}
+
+int rgrmhd_max_speed(rgrmhd_t h, double* host_out) {
+  if (!h || !host_out) return RGRMHD_E_INVALID;
+  if (!h->have_metric) return RGRMHD_E_STATE;
+  DeviceGuard guard(h->device);
+  RG_CUDA(h, cudaMemsetAsync(h->maxspeed_dev, 0, sizeof(unsigned long long), h->stream));
+  RG_CUDA(h, rg::launch_max_speed(h->G, h->maxspeed_dev, h->stream));
+  ++h->launches;
+  unsigned long long bits = 0;
+  RG_CUDA(h, cudaMemcpyAsync(&bits, h->maxspeed_dev, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
+  RG_CUDA(h, cudaStreamSynchronize(h->stream));
+  double v;
+  std::memcpy(&v, &bits, sizeof(v));
+  *host_out = v;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_get_prims(rgrmhd_t h, double* const prims[14]) {
+  if (!h || !prims) return RGRMHD_E_INVALID;
+  for (int v = 0; v < rg::NPRIM; ++v) if (!prims[v]) return RGRMHD_E_INVALID;
+  if (!h->have_prims) return RGRMHD_E_STATE;
+  DeviceGuard guard(h->device);
+  const rg::GridView& G = h->G;
+  if (G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1) {
+    RG_CUDA(h, rg::launch_ghost_fill(G, G.P, rg::NPRIM, h->stream));
+    ++h->launches;
+  }
+  int rc;
+  for (int v = 0; v < rg::NPRIM; ++v) if ((rc = copy_out(h, prims[v], G.P[v]))) return rc;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_get_cons(rgrmhd_t h, double* const cons[14]) {
+  if (!h || !cons) return RGRMHD_E_INVALID;
+  for (int v = 0; v < rg::NCONS; ++v) if (!cons[v]) return RGRMHD_E_INVALID;
+  if (!h->have_prims) return RGRMHD_E_STATE;
+  DeviceGuard guard(h->device);
+  int rc;
+  for (int v = 0; v < rg::NCONS; ++v) if ((rc = copy_out(h, cons[v], h->G.Un[v]))) return rc;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_get_stats(rgrmhd_t h, rgrmhd_stats* host_out) {
+  if (!h || !host_out) return RGRMHD_E_INVALID;
+  DeviceGuard guard(h->device);
+  rg::StatsDev s;
+  RG_CUDA(h, cudaMemcpyAsync(&s, h->stats_dev, sizeof(s), cudaMemcpyDeviceToHost, h->stream));
+  RG_CUDA(h, cudaStreamSynchronize(h->stream));
+  host_out->c2p_solves = h->solves;
+  host_out->c2p_evals = (long long)s.evals;
+  host_out->c2p_failures = (long long)s.failures;
+  host_out->floor_resets = (long long)s.floors;
+  host_out->c2p_max_evals = s.max_evals;
+  host_out->reserved = 0;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_reset_stats(rgrmhd_t h) {
+  if (!h) return RGRMHD_E_INVALID;
+  DeviceGuard guard(h->device);
+  RG_CUDA(h, cudaMemsetAsync(h->stats_dev, 0, sizeof(rg::StatsDev), h->stream));
+  h->solves = 0;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_launch_count(rgrmhd_t h, long long* host_out) {
+  if (!h || !host_out) return RGRMHD_E_INVALID;
+  *host_out = h->launches;
+  return RGRMHD_OK;
+}
+
+const char* rgrmhd_strerror(int code) {
+  switch (code) {
+    case RGRMHD_OK: return "ok";
+    case RGRMHD_E_INVALID: return "invalid argument";
+    case RGRMHD_E_STATE: return "call out of order (metric / primitives / sigma not set, or wrong sigma model)";
+    case RGRMHD_E_CUDA: return "CUDA error (see rgrmhd_last_cuda_error)";
+    case RGRMHD_E_NOMEM: return "device allocation failed";
+  }
+  return "unknown status";
+}
+
+const char* rgrmhd_last_cuda_error(rgrmhd_t h) {
+  return h ? h->last_error.c_str() : "";
+}
+
+}  // extern "C"

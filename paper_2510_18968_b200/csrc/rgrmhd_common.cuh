@@ -1,0 +1,342 @@
+// rgrmhd_common.cuh -- device-side data model and point-wise physics of the B200-native resistive
+// GRMHD step (product code; shares nothing with oracle/).
+//
+// Every function cites the passage of the paper (PAPER.md:line, equation) or the DESIGN.md reading
+// (R1..R14) it implements.  All arithmetic is FP64; nvcc may contract a*b+c into DFMA, which is the
+// only divergence from the oracle that DESIGN.md Sec. 3 allows.  No rsqrt, no pow.
+//
+// Notation: hats = undensitised conserved variables X^ = X/sqrt(gamma); vU = v^i, vD = v_i;
+// h = rho(1+eps)+p is the enthalpy density; Z = h W^2.  Symmetric tensors are stored
+// xx,xy,xz,yy,yz,zz.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace rg {
+
+enum { NPRIM = 14, NCONS = 14, NMET = 16 };
+// primitive indices
+enum { RHO = 0, PRS, VX, VY, VZ, EX, EY, EZ, BX, BY, BZ, PSI, PHI, QCH };
+// conserved indices
+enum { CD = 0, CSX, CSY, CSZ, CTAU, CEX, CEY, CEZ, CBX, CBY, CBZ, CPSI, CPHI, CQ };
+enum { MALP = 0, MBX, MBY, MBZ, MGXX, MGXY, MGXZ, MGYY, MGYZ, MGZZ, MKXX, MKXY, MKXZ, MKYY, MKYZ, MKZZ };
+enum { BC_PERIODIC = 0, BC_OUTFLOW = 1 };
+enum { SIGMA_UNIFORM = 0, SIGMA_ARRAY = 1, SIGMA_POWER_D = 2, SIGMA_ATMO = 3 };
+enum { CHARGE_FACE_OHM = 0, CHARGE_CELL_CURRENT = 1 };
+enum { RECON_MINMOD = 0, RECON_MC = 1, RECON_WENO5 = 2 };
+
+// Device view of one block: geometry, model constants and the SoA field pointers (all DEVICE memory,
+// padded layout of include/rgrmhd.h).  Passed to kernels by value as a __grid_constant__ parameter.
+struct GridView {
+  int n[3];        // interior cells
+  int np[3];       // padded cells
+  int g[3];        // ghost offset (3 for active directions, 0 for inactive)
+  int bc[3];
+  long long stride[3];
+  long long ntot;
+  double dx[3], inv_dx[3], inv_12dx[3];
+  double Gamma, sigma0, sigma_dref, kappa, rho_floor, p_atmo, tol, weno_eps;
+  int sigma_model, sigma_exp, maxit, charge_mode;
+  const double* met[NMET];
+  const double* sigma;   // SIGMA_ARRAY only, else nullptr
+  double* P[NPRIM];      // primitives of the current stage (ghosts filled by k_ghost_fill)
+  double* jc[3];         // undensitised conduction current of the current stage (reading R3)
+  double* Un[NCONS];     // U^n, overwritten with U^{n+1} by the stage-2 combine
+  double* Us[NCONS];     // stage vector U*^(2)
+  double* X1[3];         // calE^(1) (needed again by the final combine, Eq. 37)
+};
+
+struct StatsDev {
+  unsigned long long evals, failures, floors;
+  int max_evals, pad;
+};
+
+// ------------------------------------------------------------------------------------------------
+// metric algebra at one point (Eq. 1-5)
+// ------------------------------------------------------------------------------------------------
+struct Met {
+  double alpha, b[3];   // lapse, shift beta^i
+  double g[6];          // gamma_ij
+  double gi[6];         // gamma^ij
+  double sg;            // sqrt(det gamma_ij)
+};
+
+__device__ __forceinline__ constexpr int sym(int i, int j) {
+  return (i == 0) ? j : (j == 0) ? i : (i == 1) ? ((j == 1) ? 3 : 4) : ((j == 1) ? 4 : 5);
+}
+
+// sqrt(gamma) and gamma^ij = adjugate/det from gamma_ij
+__device__ __forceinline__ void met_finish(Met& m) {
+  const double gxx = m.g[0], gxy = m.g[1], gxz = m.g[2], gyy = m.g[3], gyz = m.g[4], gzz = m.g[5];
+  const double cxx = gyy * gzz - gyz * gyz;
+  const double cxy = gxz * gyz - gxy * gzz;
+  const double cxz = gxy * gyz - gxz * gyy;
+  const double det = gxx * cxx + gxy * cxy + gxz * cxz;
+  const double idet = 1.0 / det;
+  m.sg = sqrt(det);
+  m.gi[0] = cxx * idet;
+  m.gi[1] = cxy * idet;
+  m.gi[2] = cxz * idet;
+  m.gi[3] = (gxx * gzz - gxz * gxz) * idet;
+  m.gi[4] = (gxy * gxz - gxx * gyz) * idet;
+  m.gi[5] = (gxx * gyy - gxy * gxy) * idet;
+}
+
+__device__ __forceinline__ void lower(const Met& m, const double aU[3], double aD[3]) {
+  aD[0] = m.g[0] * aU[0] + m.g[1] * aU[1] + m.g[2] * aU[2];
+  aD[1] = m.g[1] * aU[0] + m.g[3] * aU[1] + m.g[4] * aU[2];
+  aD[2] = m.g[2] * aU[0] + m.g[4] * aU[1] + m.g[5] * aU[2];
+}
+__device__ __forceinline__ void raise(const Met& m, const double aD[3], double aU[3]) {
+  aU[0] = m.gi[0] * aD[0] + m.gi[1] * aD[1] + m.gi[2] * aD[2];
+  aU[1] = m.gi[1] * aD[0] + m.gi[3] * aD[1] + m.gi[4] * aD[2];
+  aU[2] = m.gi[2] * aD[0] + m.gi[4] * aD[1] + m.gi[5] * aD[2];
+}
+__device__ __forceinline__ double dot3(const double a[3], const double b[3]) {
+  return a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+}
+// [ijk] a_j b_k (no metric factor)
+__device__ __forceinline__ void cross_raw(const double a[3], const double b[3], double c[3]) {
+  c[0] = a[1] * b[2] - a[2] * b[1];
+  c[1] = a[2] * b[0] - a[0] * b[2];
+  c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+__device__ __forceinline__ void load_met_cell(const GridView& G, long long c, Met& m) {
+  m.alpha = __ldg(G.met[MALP] + c);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) m.b[i] = __ldg(G.met[MBX + i] + c);
+#pragma unroll
+  for (int q = 0; q < 6; ++q) m.g[q] = __ldg(G.met[MGXX + q] + c);
+  met_finish(m);
+}
+// reading R2: face metric = arithmetic mean of alpha, beta^i, gamma_ij of the two adjacent centres;
+// sqrt(gamma), gamma^ij from the averaged gamma_ij
+__device__ __forceinline__ void load_met_face(const GridView& G, long long cL, long long cR, Met& m) {
+  m.alpha = 0.5 * (__ldg(G.met[MALP] + cL) + __ldg(G.met[MALP] + cR));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) m.b[i] = 0.5 * (__ldg(G.met[MBX + i] + cL) + __ldg(G.met[MBX + i] + cR));
+#pragma unroll
+  for (int q = 0; q < 6; ++q) m.g[q] = 0.5 * (__ldg(G.met[MGXX + q] + cL) + __ldg(G.met[MGXX + q] + cR));
+  met_finish(m);
+}
+
+// ------------------------------------------------------------------------------------------------
+// A18. conductivity models (Eq. 52; Eq. 61; reading R13), Dhat = D/sqrt(gamma)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double sigma_of(const GridView& G, double Dhat, long long c) {
+  switch (G.sigma_model) {
+    case SIGMA_UNIFORM: return G.sigma0;
+    case SIGMA_ARRAY: return __ldg(G.sigma + c);
+    case SIGMA_POWER_D: {
+      const double x = Dhat / G.sigma_dref;
+      double r = 1.0;
+      for (int i = 0; i < G.sigma_exp; ++i) r *= x;   // integer exponent by multiplication, no pow
+      return G.sigma0 * r;
+    }
+    case SIGMA_ATMO: {
+      const double x = fmax(1.0 - G.sigma_dref / Dhat, 0.0);
+      return G.sigma0 * x * x;
+    }
+  }
+  return 0.0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a0. primitive -> conserved at one point (Eq. 22-24; Eq. 28; EOS Eq. 49)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void prim2cons(const Met& m, double Gamma, const double P[NPRIM], double U[NCONS]) {
+  const double rho = P[RHO], p = P[PRS];
+  const double vU[3] = {P[VX], P[VY], P[VZ]}, EU[3] = {P[EX], P[EY], P[EZ]}, BU[3] = {P[BX], P[BY], P[BZ]};
+  double vD[3], ED[3], BD[3], ExB[3];
+  lower(m, vU, vD); lower(m, EU, ED); lower(m, BU, BD);
+  const double v2 = dot3(vU, vD);
+  const double W = 1.0 / sqrt(1.0 - v2);
+  const double h = rho + Gamma / (Gamma - 1.0) * p;            // rho(1+eps)+p with Eq. 49
+  const double E2 = dot3(EU, ED), B2 = dot3(BU, BD);
+  cross_raw(EU, BU, ExB);                                      // eps_ijk E^j B^k = sg [ijk] E^j B^k
+  const double sg = m.sg, hW2 = h * W * W;
+  U[CD] = sg * rho * W;                                        // Eq. 22
+#pragma unroll
+  for (int i = 0; i < 3; ++i) U[CSX + i] = sg * (hW2 * vD[i] + sg * ExB[i]);   // Eq. 24
+  U[CTAU] = sg * (hW2 - p + 0.5 * (E2 + B2)) - U[CD];          // Eq. 23
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { U[CEX + i] = sg * EU[i]; U[CBX + i] = sg * BU[i]; }   // Eq. 28
+  U[CPSI] = sg * P[PSI]; U[CPHI] = sg * P[PHI]; U[CQ] = sg * P[QCH];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3 (first half). U and F^k of one state at one face: Eq. 27 in reading R1
+//   T^k_j = h W^2 v^k v_j + delta^k_j p - E^k E_j - B^k B_j + delta^k_j (E^2+B^2)/2
+//   F(D)=(alpha v^k - beta^k) D ; F(S_j)=alpha sg T^k_j - beta^k S_j ; F(tau)=alpha(S^k - v^k D) - beta^k tau
+//   F(calB^i)= alpha([ikj] E_j + g^ik Phi) - beta^k calB^i ; F(calE^i)=-alpha([ikj] B_j - g^ik Psi) - beta^k calE^i
+//   F(Phi)=alpha calB^k - beta^k Phi ; F(Psi)=alpha calE^k - beta^k Psi
+//   F(calQ)=alpha J^k - beta^k calQ, J^k = calQ v^k + Jc^k (Eq. 29; reading R3)
+// ------------------------------------------------------------------------------------------------
+template <int K, int CHARGE>
+__device__ __forceinline__ void state_flux(const Met& m, double Gamma, const double P[NPRIM], double sigma,
+                                           double jck, double U[NCONS], double F[NCONS]) {
+  const double rho = P[RHO], p = P[PRS];
+  const double vU[3] = {P[VX], P[VY], P[VZ]}, EU[3] = {P[EX], P[EY], P[EZ]}, BU[3] = {P[BX], P[BY], P[BZ]};
+  double vD[3], ED[3], BD[3], ExB[3];
+  lower(m, vU, vD); lower(m, EU, ED); lower(m, BU, BD);
+  const double v2 = dot3(vU, vD);
+  const double W = 1.0 / sqrt(1.0 - v2);
+  const double h = rho + Gamma / (Gamma - 1.0) * p;
+  const double E2 = dot3(EU, ED), B2 = dot3(BU, BD);
+  cross_raw(EU, BU, ExB);
+  const double sg = m.sg, hW2 = h * W * W, a = m.alpha, bk = m.b[K];
+  const double pem = 0.5 * (E2 + B2);
+  U[CD] = sg * rho * W;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) U[CSX + i] = sg * (hW2 * vD[i] + sg * ExB[i]);
+  U[CTAU] = sg * (hW2 - p + pem) - U[CD];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { U[CEX + i] = sg * EU[i]; U[CBX + i] = sg * BU[i]; }
+  U[CPSI] = sg * P[PSI]; U[CPHI] = sg * P[PHI]; U[CQ] = sg * P[QCH];
+
+  F[CD] = (a * vU[K] - bk) * U[CD];
+  const double asg = a * sg;
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    double Tkj = hW2 * vU[K] * vD[j] - EU[K] * ED[j] - BU[K] * BD[j];
+    if (j == K) Tkj += p + pem;
+    F[CSX + j] = asg * Tkj - bk * U[CSX + j];
+  }
+  const double SUk = m.gi[sym(K, 0)] * U[CSX] + m.gi[sym(K, 1)] * U[CSY] + m.gi[sym(K, 2)] * U[CSZ];
+  F[CTAU] = a * (SUk - vU[K] * U[CD]) - bk * U[CTAU];
+  // [ikj] X_j: for i = K zero; i = K+1: [K+1,K,K+2] = -1 -> -X_{K+2}; i = K+2: [K+2,K,K+1] = +1 -> +X_{K+1}
+  constexpr int K1 = (K + 1) % 3, K2 = (K + 2) % 3;
+  double curlE[3], curlB[3];
+  curlE[K] = 0.0;      curlB[K] = 0.0;
+  curlE[K1] = -ED[K2]; curlB[K1] = -BD[K2];
+  curlE[K2] = ED[K1];  curlB[K2] = BD[K1];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    F[CBX + i] = a * (curlE[i] + m.gi[sym(i, K)] * U[CPHI]) - bk * U[CBX + i];
+    F[CEX + i] = -a * (curlB[i] - m.gi[sym(i, K)] * U[CPSI]) - bk * U[CEX + i];
+  }
+  F[CPHI] = a * U[CBX + K] - bk * U[CPHI];
+  F[CPSI] = a * U[CEX + K] - bk * U[CPSI];
+  double Jck;
+  if (CHARGE == CHARGE_FACE_OHM) {
+    double vxB[3];
+    cross_raw(vD, BD, vxB);                                 // (v x B)^i = [ijk] v_j B_k / sg
+    const double vE = dot3(EU, vD);
+    Jck = W * sigma * (U[CEX + K] + vxB[K] - vE * sg * vU[K]);   // Eq. 29 densitised: sg (v x B)^k = [kij] v_i B_j
+  } else {
+    Jck = sg * jck;
+  }
+  F[CQ] = a * (U[CQ] * vU[K] + Jck) - bk * U[CQ];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2. reconstruction of one variable from the 5-cell stencil centred on a cell (reading R4).
+//     lo = value at the cell's lower face (right state of face i-1/2), hi = at its upper face.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double minmod2(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  return copysign(fmin(fabs(a), fabs(b)), a);
+}
+__device__ __forceinline__ double minmod3(double a, double b, double c) {
+  if (a > 0.0 && b > 0.0 && c > 0.0) return fmin(a, fmin(b, c));
+  if (a < 0.0 && b < 0.0 && c < 0.0) return fmax(a, fmax(b, c));
+  return 0.0;
+}
+// Jiang-Shu smoothness indicators of the stencil u0..u4 (shared by both faces of the centre cell)
+__device__ __forceinline__ void weno5_beta(double u0, double u1, double u2, double u3, double u4, double eps_w,
+                                           double& b0, double& b1, double& b2) {
+  const double d0 = u0 - 2.0 * u1 + u2, e0 = u0 - 4.0 * u1 + 3.0 * u2;
+  const double d1 = u1 - 2.0 * u2 + u3, e1 = u1 - u3;
+  const double d2 = u2 - 2.0 * u3 + u4, e2 = 3.0 * u2 - 4.0 * u3 + u4;
+  b0 = eps_w + (13.0 / 12.0 * d0 * d0 + 0.25 * e0 * e0);
+  b1 = eps_w + (13.0 / 12.0 * d1 * d1 + 0.25 * e1 * e1);
+  b2 = eps_w + (13.0 / 12.0 * d2 * d2 + 0.25 * e2 * e2);
+}
+// value at the +1/2 face of the centre cell u2; b0,b1,b2 = eps_w + beta_k of the stencils
+// {u0,u1,u2},{u1,u2,u3},{u2,u3,u4}.  Weights d_k/b_k^2 with d = (0.1,0.6,0.3), normalised; written in
+// product form (one division): w_k ~ d_k (b_l b_m)^2.
+__device__ __forceinline__ double weno5_eval(double u0, double u1, double u2, double u3, double u4,
+                                             double b0, double b1, double b2) {
+  const double q0 = 2.0 * u0 - 7.0 * u1 + 11.0 * u2;
+  const double q1 = -u1 + 5.0 * u2 + 2.0 * u3;
+  const double q2 = 2.0 * u2 + 5.0 * u3 - u4;
+  const double p12 = b1 * b2, p02 = b0 * b2, p01 = b0 * b1;
+  const double a0 = 0.1 * (p12 * p12), a1 = 0.6 * (p02 * p02), a2 = 0.3 * (p01 * p01);
+  return (a0 * q0 + a1 * q1 + a2 * q2) / (6.0 * (a0 + a1 + a2));
+}
+template <int RECON>
+__device__ __forceinline__ void recon_cell(double eps_w, double um2, double um1, double u0, double up1, double up2,
+                                           double& lo, double& hi) {
+  if (RECON == RECON_WENO5) {
+    double b0, b1, b2;
+    weno5_beta(um2, um1, u0, up1, up2, eps_w, b0, b1, b2);
+    hi = weno5_eval(um2, um1, u0, up1, up2, b0, b1, b2);
+    lo = weno5_eval(up2, up1, u0, um1, um2, b2, b1, b0);      // mirror image
+  } else {
+    const double a = u0 - um1, b = up1 - u0;
+    const double slope = (RECON == RECON_MINMOD) ? minmod2(a, b) : minmod3(2.0 * a, 2.0 * b, 0.5 * (a + b));
+    hi = u0 + 0.5 * slope;
+    lo = u0 - 0.5 * slope;
+  }
+}
+// one-sided versions (a face needs `hi` of its left cell and `lo` of its right cell)
+template <int RECON>
+__device__ __forceinline__ double recon_hi(double eps_w, double um2, double um1, double u0, double up1, double up2) {
+  if (RECON == RECON_WENO5) {
+    double b0, b1, b2;
+    weno5_beta(um2, um1, u0, up1, up2, eps_w, b0, b1, b2);
+    return weno5_eval(um2, um1, u0, up1, up2, b0, b1, b2);
+  } else {
+    const double a = u0 - um1, b = up1 - u0;
+    const double slope = (RECON == RECON_MINMOD) ? minmod2(a, b) : minmod3(2.0 * a, 2.0 * b, 0.5 * (a + b));
+    return u0 + 0.5 * slope;
+  }
+}
+template <int RECON>
+__device__ __forceinline__ double recon_lo(double eps_w, double um2, double um1, double u0, double up1, double up2) {
+  if (RECON == RECON_WENO5) {
+    double b0, b1, b2;
+    weno5_beta(um2, um1, u0, up1, up2, eps_w, b0, b1, b2);
+    return weno5_eval(up2, up1, u0, um1, um2, b2, b1, b0);
+  } else {
+    const double a = u0 - um1, b = up1 - u0;
+    const double slope = (RECON == RECON_MINMOD) ? minmod2(a, b) : minmod3(2.0 * a, 2.0 * b, 0.5 * (a + b));
+    return u0 - 0.5 * slope;
+  }
+}
+
+// reading R4: limit |v| of a face state with the face metric
+__device__ __forceinline__ void limit_velocity(const Met& m, double P[NPRIM]) {
+  const double vU[3] = {P[VX], P[VY], P[VZ]};
+  double vD[3];
+  lower(m, vU, vD);
+  const double v2 = dot3(vU, vD), v2max = 1.0 - 1e-10;
+  if (v2 >= v2max) {
+    const double f = sqrt(v2max / v2);
+    P[VX] *= f; P[VY] *= f; P[VZ] *= f;
+  }
+}
+
+// a3 (second half). HLLE combination (Eq. 30; reading R6)
+template <int K, int CHARGE>
+__device__ __forceinline__ void hlle(const Met& mf, double Gamma, double PL[NPRIM], double PR[NPRIM],
+                                     double sigL, double sigR, double jL, double jR, double Fh[NCONS]) {
+  limit_velocity(mf, PL);
+  limit_velocity(mf, PR);
+  double UL[NCONS], FL[NCONS], UR[NCONS], FR[NCONS];
+  state_flux<K, CHARGE>(mf, Gamma, PL, sigL, jL, UL, FL);
+  state_flux<K, CHARGE>(mf, Gamma, PR, sigR, jR, UR, FR);
+  const double c = mf.alpha * sqrt(mf.gi[sym(K, K)]);
+  const double lp = fmax(0.0, c - mf.b[K]);
+  const double lm = fmin(0.0, -c - mf.b[K]);
+  const double inv = 1.0 / (lp - lm), lplm = lp * lm;
+#pragma unroll
+  for (int v = 0; v < NCONS; ++v) Fh[v] = (lp * FL[v] - lm * FR[v] + lplm * (UR[v] - UL[v])) * inv;
+}
+
+__device__ __forceinline__ long long cell_index(const GridView& G, int i, int j, int k) {
+  return (long long)(i + G.g[0]) + G.stride[1] * (long long)(j + G.g[1]) + G.stride[2] * (long long)(k + G.g[2]);
+}
+
+}  // namespace rg
