@@ -142,6 +142,19 @@ int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant);
 /* Kernel launches enqueued by this handle since create (bench.py's "gpu_launches"). */
 int rgrmhd_launch_count(rgrmhd_t h, long long* host_out);
 
+/* Per-kernel device timing (bench.py's roofline object).  While enabled, rgrmhd_step brackets every
+ * kernel it launches with CUDA events on the handle's stream; rgrmhd_get_timing synchronises, adds the
+ * elapsed milliseconds and launch counts since the last call into ms[k] / launches[k] (OVERWRITING
+ * them) for the kernel classes below, and forgets the events. */
+enum { RGRMHD_K_C2P = 0, RGRMHD_K_GHOST = 1, RGRMHD_K_RHS = 2, RGRMHD_K_COUNT = 3 };
+int rgrmhd_set_timing(rgrmhd_t h, int enable);
+int rgrmhd_get_timing(rgrmhd_t h, double ms[RGRMHD_K_COUNT], long long launches[RGRMHD_K_COUNT]);
+
+/* Measurement aid for the FP64 roofline denominator: runs a register-resident
+ * DFMA kernel (8 independent chains per thread, every SM full) on `device` and writes the best of
+ * `repeats` timings as TFLOP/s (FMA = 2 flops) to *tflops_out.  Synchronises the device. */
+int rgrmhd_measure_fp64_peak(int device, int repeats, double* tflops_out);
+
 const char* rgrmhd_strerror(int code);
 const char* rgrmhd_last_cuda_error(rgrmhd_t h);
 

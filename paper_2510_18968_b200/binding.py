@@ -23,7 +23,10 @@ NMETRIC = 16
 SYMBOLS = ["rgrmhd_params_default", "rgrmhd_create", "rgrmhd_destroy", "rgrmhd_set_stream", "rgrmhd_set_metric",
            "rgrmhd_set_sigma", "rgrmhd_set_prims", "rgrmhd_step", "rgrmhd_max_speed", "rgrmhd_get_prims",
            "rgrmhd_get_cons", "rgrmhd_get_stats", "rgrmhd_reset_stats", "rgrmhd_set_rhs_variant",
-           "rgrmhd_launch_count", "rgrmhd_strerror", "rgrmhd_last_cuda_error"]
+           "rgrmhd_launch_count", "rgrmhd_set_timing", "rgrmhd_get_timing", "rgrmhd_measure_fp64_peak",
+           "rgrmhd_strerror", "rgrmhd_last_cuda_error"]
+
+KERNEL_CLASSES = ("c2p", "ghost", "rhs")
 
 
 class Params(C.Structure):
@@ -70,6 +73,9 @@ def load() -> C.CDLL:
         L.rgrmhd_reset_stats.argtypes = [vp]
         L.rgrmhd_set_rhs_variant.argtypes = [vp, C.c_int]
         L.rgrmhd_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.rgrmhd_set_timing.argtypes = [vp, C.c_int]
+        L.rgrmhd_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.rgrmhd_measure_fp64_peak.argtypes = [C.c_int, C.c_int, dp]
         L.rgrmhd_strerror.argtypes = [C.c_int]
         L.rgrmhd_strerror.restype = C.c_char_p
         L.rgrmhd_last_cuda_error.argtypes = [vp]
@@ -206,10 +212,27 @@ class Rgrmhd:
     def set_rhs_variant(self, variant: int):
         self._check(self.L.rgrmhd_set_rhs_variant(self.h, int(variant)), "rgrmhd_set_rhs_variant")
 
+    def set_timing(self, enable: bool):
+        self._check(self.L.rgrmhd_set_timing(self.h, int(bool(enable))), "rgrmhd_set_timing")
+
+    def get_timing(self) -> dict:
+        """{class: (milliseconds, launches)} accumulated since the last call."""
+        ms = (C.c_double * 3)(); ln = (C.c_longlong * 3)()
+        self._check(self.L.rgrmhd_get_timing(self.h, ms, ln), "rgrmhd_get_timing")
+        return {k: (ms[i], ln[i]) for i, k in enumerate(KERNEL_CLASSES)}
+
     def launch_count(self) -> int:
         out = C.c_longlong()
         self._check(self.L.rgrmhd_launch_count(self.h, C.byref(out)), "rgrmhd_launch_count")
         return out.value
+
+
+def measure_fp64_peak(device: int = 0, repeats: int = 5) -> float:
+    out = C.c_double()
+    rc = load().rgrmhd_measure_fp64_peak(int(device), int(repeats), C.byref(out))
+    if rc != 0:
+        raise RgrmhdError("rgrmhd_measure_fp64_peak", rc)
+    return out.value
 
 
 def from_workload(w, fields: Optional[dict] = None, n=None, bc=None, device: int = 0, **over) -> Rgrmhd:

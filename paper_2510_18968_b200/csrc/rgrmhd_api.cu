@@ -6,6 +6,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/rgrmhd.h"
 #include "rgrmhd_common.cuh"
@@ -34,6 +35,9 @@ struct rgrmhd_s {
   long long launches = 0;
   bool have_metric = false, have_prims = false, have_sigma = false;
   int rhs_variant = 0;               // 0 = tiled (default), 1 = simple
+  bool timing = false;
+  struct Timed { int cls; cudaEvent_t a, b; };
+  std::vector<Timed> timed;
   std::string last_error;
 };
 
@@ -167,6 +171,7 @@ int rgrmhd_destroy(rgrmhd_t h) {
   {
     DeviceGuard guard(h->device);
     cudaStreamSynchronize(h->stream);
+    for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(h->slab);
     cudaFree(h->stats_dev);
   }
@@ -257,16 +262,30 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   auto rhs = [&](int stage) {
     return tiled ? rg::launch_rhs_tiled(G, dt, stage, recon, st) : rg::launch_rhs_simple(G, dt, stage, recon, st);
   };
+  // optional per-kernel event bracket (rgrmhd_set_timing)
+  auto timed = [&](int cls, auto&& launch) -> cudaError_t {
+    if (!h->timing) return launch();
+    rgrmhd_s::Timed t{cls, nullptr, nullptr};
+    cudaError_t e = cudaEventCreate(&t.a);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&t.b);
+    if (e != cudaSuccess) { cudaEventDestroy(t.a); return e; }
+    cudaEventRecord(t.a, st);
+    e = launch();
+    cudaEventRecord(t.b, st);
+    h->timed.push_back(t);
+    return e;
+  };
   // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n
-  RG_CUDA(h, rg::launch_c2p(G, G.Un, G.X1, gam * dt, false, h->stats_dev, st));
-  RG_CUDA(h, rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st));
-  RG_CUDA(h, rhs(1));                                         // -> U*2 (Eq. 36)
+  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, G.Un, G.X1, gam * dt, false, h->stats_dev, st); }));
+  if (any_active) RG_CUDA(h, timed(RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  RG_CUDA(h, timed(RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
   // stage 2 (Eq. 36)
-  RG_CUDA(h, rg::launch_c2p(G, G.Us, nullptr, gam * dt, false, h->stats_dev, st));
-  RG_CUDA(h, rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st));
-  RG_CUDA(h, rhs(2));                                         // -> U^{n+1} (Eq. 37)
+  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, G.Us, nullptr, gam * dt, false, h->stats_dev, st); }));
+  if (any_active) RG_CUDA(h, timed(RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  RG_CUDA(h, timed(RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
   // recovery of the new state at fixed calE (reading R12)
-  RG_CUDA(h, rg::launch_c2p(G, G.Un, nullptr, 0.0, true, h->stats_dev, st));
+  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, G.Un, nullptr, 0.0, true, h->stats_dev, st); }));
   h->solves += 3 * nint;
   h->launches += 5 + (any_active ? 2 : 0);
   return RGRMHD_OK;
@@ -333,6 +352,66 @@ int rgrmhd_reset_stats(rgrmhd_t h) {
   DeviceGuard guard(h->device);
   RG_CUDA(h, cudaMemsetAsync(h->stats_dev, 0, sizeof(rg::StatsDev), h->stream));
   h->solves = 0;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_set_timing(rgrmhd_t h, int enable) {
+  if (!h) return RGRMHD_E_INVALID;
+  h->timing = enable != 0;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_get_timing(rgrmhd_t h, double ms[RGRMHD_K_COUNT], long long launches[RGRMHD_K_COUNT]) {
+  if (!h || !ms || !launches) return RGRMHD_E_INVALID;
+  DeviceGuard guard(h->device);
+  for (int k = 0; k < RGRMHD_K_COUNT; ++k) { ms[k] = 0.0; launches[k] = 0; }
+  RG_CUDA(h, cudaStreamSynchronize(h->stream));
+  for (auto& t : h->timed) {
+    float f = 0.f;
+    if (cudaEventElapsedTime(&f, t.a, t.b) == cudaSuccess) { ms[t.cls] += f; launches[t.cls] += 1; }
+    cudaEventDestroy(t.a); cudaEventDestroy(t.b);
+  }
+  h->timed.clear();
+  return RGRMHD_OK;
+}
+
+namespace {
+__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a, double b) {
+  double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int i = 0; i < iters; ++i) {
+    x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+    x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+  }
+  const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == 12345.678) out[0] = s;   // never true for the arguments used; keeps the chains alive
+}
+}  // namespace
+
+int rgrmhd_measure_fp64_peak(int device, int repeats, double* tflops_out) {
+  if (!tflops_out || repeats < 1) return RGRMHD_E_INVALID;
+  DeviceGuard guard(device);
+  if (!guard.ok) return RGRMHD_E_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return RGRMHD_E_CUDA;
+  double* out = nullptr;
+  if (cudaMalloc((void**)&out, sizeof(double)) != cudaSuccess) return RGRMHD_E_NOMEM;
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 1 << 14;
+  double best = 0.0;
+  for (int r = 0; r < repeats + 1; ++r) {
+    cudaEventRecord(a);
+    k_dfma_peak<<<blocks, threads>>>(out, iters, 0.999999, 1e-9);
+    cudaEventRecord(b);
+    if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(out); return RGRMHD_E_CUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    const double tf = 2.0 * 8.0 * (double)iters * blocks * threads / (ms * 1e-3) * 1e-12;
+    if (r > 0 && tf > best) best = tf;   // first launch is warm-up
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  cudaFree(out);
+  *tflops_out = best;
   return RGRMHD_OK;
 }
 
