@@ -322,17 +322,22 @@ __device__ __forceinline__ void limit_velocity(const Met& m, double P[NPRIM]) {
 template <int K, int CHARGE>
 __device__ __forceinline__ void hlle(const Met& mf, double Gamma, double PL[NPRIM], double PR[NPRIM],
                                      double sigL, double sigR, double jL, double jR, double Fh[NCONS]) {
-  limit_velocity(mf, PL);
-  limit_velocity(mf, PR);
-  double UL[NCONS], FL[NCONS], UR[NCONS], FR[NCONS];
-  state_flux<K, CHARGE>(mf, Gamma, PL, sigL, jL, UL, FL);
-  state_flux<K, CHARGE>(mf, Gamma, PR, sigR, jR, UR, FR);
+  // F = (lp FL - lm FR + lp lm (UR - UL))/(lp - lm), accumulated state by state so that only one
+  // state's (U, F) pair is live at a time
   const double c = mf.alpha * sqrt(mf.gi[sym(K, K)]);
   const double lp = fmax(0.0, c - mf.b[K]);
   const double lm = fmin(0.0, -c - mf.b[K]);
-  const double inv = 1.0 / (lp - lm), lplm = lp * lm;
+  const double inv = 1.0 / (lp - lm);
+  const double cL = lp * inv, cR = -lm * inv, cU = lp * lm * inv;
+  double U[NCONS], F[NCONS];
+  limit_velocity(mf, PL);
+  state_flux<K, CHARGE>(mf, Gamma, PL, sigL, jL, U, F);
 #pragma unroll
-  for (int v = 0; v < NCONS; ++v) Fh[v] = (lp * FL[v] - lm * FR[v] + lplm * (UR[v] - UL[v])) * inv;
+  for (int v = 0; v < NCONS; ++v) Fh[v] = cL * F[v] - cU * U[v];
+  limit_velocity(mf, PR);
+  state_flux<K, CHARGE>(mf, Gamma, PR, sigR, jR, U, F);
+#pragma unroll
+  for (int v = 0; v < NCONS; ++v) Fh[v] += cR * F[v] + cU * U[v];
 }
 
 __device__ __forceinline__ long long cell_index(const GridView& G, int i, int j, int k) {
