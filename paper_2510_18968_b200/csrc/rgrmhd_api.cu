@@ -18,6 +18,8 @@ cudaError_t launch_prim2cons(const GridView& G, cudaStream_t st);
 cudaError_t launch_rhs_simple(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 cudaError_t launch_rhs_tiled(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 bool rhs_tiled_supported(const GridView& G);
+cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
+bool rhs_pencil_supported(const GridView& G);
 cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, cudaStream_t st);
 cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, cudaStream_t st);
 }  // namespace rg
@@ -34,7 +36,7 @@ struct rgrmhd_s {
   long long solves = 0;              // host-side count of cell solves enqueued
   long long launches = 0;
   bool have_metric = false, have_prims = false, have_sigma = false;
-  int rhs_variant = 0;               // 0 = tiled (default), 1 = simple
+  int rhs_variant = 0;               // 0 = pencil (default), 1 = simple, 2 = tiled (first generation)
   bool timing = false;
   struct Timed { int cls; cudaEvent_t a, b; };
   std::vector<Timed> timed;
@@ -186,7 +188,7 @@ int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream) {
 }
 
 int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant) {
-  if (!h || variant < 0 || variant > 1) return RGRMHD_E_INVALID;
+  if (!h || variant < 0 || variant > 2) return RGRMHD_E_INVALID;
   h->rhs_variant = variant;
   return RGRMHD_OK;
 }
@@ -258,9 +260,12 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   for (int q = 0; q < 3; ++q) ghost_fields[rg::NPRIM + q] = G.jc[q];
   const int nghost_fields = rg::NPRIM + (G.charge_mode == rg::CHARGE_CELL_CURRENT ? 3 : 0);
   const bool any_active = G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1;
-  const bool tiled = h->rhs_variant == 0 && rg::rhs_tiled_supported(G);
+  const bool pencil = h->rhs_variant == 0 && rg::rhs_pencil_supported(G);
+  const bool tiled = h->rhs_variant == 2 && rg::rhs_tiled_supported(G);
   auto rhs = [&](int stage) {
-    return tiled ? rg::launch_rhs_tiled(G, dt, stage, recon, st) : rg::launch_rhs_simple(G, dt, stage, recon, st);
+    return pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, st)
+         : tiled  ? rg::launch_rhs_tiled(G, dt, stage, recon, st)
+                  : rg::launch_rhs_simple(G, dt, stage, recon, st);
   };
   // optional per-kernel event bracket (rgrmhd_set_timing)
   auto timed = [&](int cls, auto&& launch) -> cudaError_t {

@@ -1,0 +1,402 @@
+// rgrmhd_rhs_pencil.cu -- the production RHS kernel (a2-a5): reconstruct + HLLE + flux divergence +
+// explicit sources + IMEX stage combine in ONE launch.  Face states and fluxes never leave the SM.
+//
+// Decomposition ("pencil-tiled"): a CTA owns a TX x TY (x, y) tile of z-pencils and marches CZ planes
+// along z; one thread = one cell of the current plane.  Per plane, for each direction K (x, y, z):
+//   a2  every thread reconstructs ITS OWN CELL along K for all 15 variables: the smoothness
+//       indicators are computed once and give both the value at the cell's lower face (kept in
+//       registers: the right state of that face) and at its upper face (the left state of the next
+//       face).  The upper-face values are handed to the neighbouring thread through shared memory
+//       (x, y) or kept in a thread-private shared-memory slot for the next plane (z).
+//   a3  every thread solves the HLLE problem at its cell's lower face (x, y) / upper face (z); the
+//       flux goes to shared memory (aliasing the exchange buffer) and each cell differences its own
+//       and its neighbour's flux.  No face is solved twice except the TX + TY faces on the tile's
+//       upper x / y edge, which one warp each handles in an extra pass (their reconstruction halo:
+//       two more partial warps).
+//   a4, a5  geometric sources, stage combine, one store of U*2 / U^{n+1}.
+// The three directions run through ONE copy of the reconstruction and Riemann code: direction K is a
+// run-time cyclic rotation of the vector/tensor components (cyclic permutations keep the Levi-Civita
+// sign, so Eq. 27 is form invariant), realised for free as index arithmetic on pointer tables and
+// shared-memory planes.  This keeps the kernel ~4x smaller than the fully templated version, whose
+// instruction-cache misses dominated its stall profile (profiles/r01_rhs_tiled_ncu.md).
+// Stencils are read straight from global memory (x: coalesced rows, L1; y: L1; z: L2).
+#include "rgrmhd_rhs.cuh"
+
+namespace rg {
+
+namespace {
+constexpr int TX = 32, TY = 8, NT = TX * TY;
+constexpr int EXW = TX + 1, EXH = TY + 1, EXP = EXW * EXH;
+constexpr int NVR = 15;   // 14 primitives + the normal component of the conduction current (reading R3)
+
+struct PencilTabs {
+  const double* P[3][NVR];   // rotated order: rho, p, v^K v^K1 v^K2, E.., B.., psi, phi, q, jc^K
+  const double* M[3][8];     // alpha, beta^K, gamma rotated: 00 01 02 11 12 22 (0 = K, 1 = K+1, 2 = K+2)
+  int nat[3][NCONS];         // rotated conserved index -> natural conserved index
+};
+
+struct Smem {
+  double ex[NVR][EXP];       // upper-face states of the tile's cells (+ lower halo); later the face fluxes
+  double exlo[NVR][TX];      // lower-face states of the upper-halo cells
+  double exhi[NVR][TX];      // upper-face states of the last interior row/column (left states of the edge faces)
+  double chi[2][NVR][NT];    // z: upper-face states of the current plane (ping-pong), then the z flux
+};
+
+struct FaceMet {
+  double alpha, b0, g[6], gi0[3], sg;
+};
+
+// reading R2: face metric = arithmetic mean of the two adjacent centres; sqrt(gamma) and the K-row of
+// gamma^ij from the averaged gamma_ij (rotated components)
+__device__ __forceinline__ void load_face_met(const PencilTabs& T, int K, long long cl, long long cr, FaceMet& m) {
+  m.alpha = 0.5 * (__ldg(T.M[K][0] + cl) + __ldg(T.M[K][0] + cr));
+  m.b0 = 0.5 * (__ldg(T.M[K][1] + cl) + __ldg(T.M[K][1] + cr));
+#pragma unroll
+  for (int q = 0; q < 6; ++q) m.g[q] = 0.5 * (__ldg(T.M[K][2 + q] + cl) + __ldg(T.M[K][2 + q] + cr));
+  const double c00 = m.g[3] * m.g[5] - m.g[4] * m.g[4];
+  const double c01 = m.g[2] * m.g[4] - m.g[1] * m.g[5];
+  const double c02 = m.g[1] * m.g[4] - m.g[2] * m.g[3];
+  const double det = m.g[0] * c00 + m.g[1] * c01 + m.g[2] * c02;
+  const double idet = 1.0 / det;
+  m.sg = sqrt(det);
+  m.gi0[0] = c00 * idet; m.gi0[1] = c01 * idet; m.gi0[2] = c02 * idet;
+}
+
+// a3, one state.  X = (rho, p, v[3], E[3], B[3], psi, phi, q, jc^0) in the rotated frame (0 = face normal).
+// Adds wa*G + wu*U to Fh, where F = alpha G - beta^0 U is Eq. 27 (reading R1), i.e. the
+// state's share w F + sd U of the HLLE flux with wa = w alpha, wu = sd - w beta^0.
+template <int CHARGE, bool FIRST>
+__device__ __forceinline__ void half_flux(const FaceMet& m, double Gamma, const double X[NVR], double sigma,
+                                          double wa, double wu, double Fh[NCONS]) {
+  const double rho = X[0], p = X[1];
+  double v[3] = {X[2], X[3], X[4]};
+  const double E[3] = {X[5], X[6], X[7]}, B[3] = {X[8], X[9], X[10]};
+  double vD[3];
+  vD[0] = m.g[0] * v[0] + m.g[1] * v[1] + m.g[2] * v[2];
+  vD[1] = m.g[1] * v[0] + m.g[3] * v[1] + m.g[4] * v[2];
+  vD[2] = m.g[2] * v[0] + m.g[4] * v[1] + m.g[5] * v[2];
+  double vsq = v[0] * vD[0] + v[1] * vD[1] + v[2] * vD[2];
+  const double v2max = 1.0 - 1e-10;
+  if (vsq >= v2max) {   // reading R4: limit |v| of a face state with the face metric
+    const double f = sqrt(v2max / vsq);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { v[a] *= f; vD[a] *= f; }
+    vsq = v[0] * vD[0] + v[1] * vD[1] + v[2] * vD[2];
+  }
+  const double ED[3] = {m.g[0] * E[0] + m.g[1] * E[1] + m.g[2] * E[2], m.g[1] * E[0] + m.g[3] * E[1] + m.g[4] * E[2],
+                        m.g[2] * E[0] + m.g[4] * E[1] + m.g[5] * E[2]};
+  const double BD[3] = {m.g[0] * B[0] + m.g[1] * B[1] + m.g[2] * B[2], m.g[1] * B[0] + m.g[3] * B[1] + m.g[4] * B[2],
+                        m.g[2] * B[0] + m.g[4] * B[1] + m.g[5] * B[2]};
+  const double W = 1.0 / sqrt(1.0 - vsq);
+  const double h = rho + Gamma / (Gamma - 1.0) * p;              // rho(1+eps)+p with Eq. 49
+  const double hW2 = h * W * W;
+  const double pem = 0.5 * ((E[0] * ED[0] + E[1] * ED[1] + E[2] * ED[2]) + (B[0] * BD[0] + B[1] * BD[1] + B[2] * BD[2]));
+  const double sg = m.sg;
+  const double ExB[3] = {E[1] * B[2] - E[2] * B[1], E[2] * B[0] - E[0] * B[2], E[0] * B[1] - E[1] * B[0]};
+  double U[NCONS], Gf[NCONS];
+  U[CD] = sg * rho * W;                                          // Eq. 22
+#pragma unroll
+  for (int a = 0; a < 3; ++a) U[CSX + a] = sg * (hW2 * vD[a] + sg * ExB[a]);   // Eq. 24
+  U[CTAU] = sg * (hW2 - p + pem) - U[CD];                        // Eq. 23
+#pragma unroll
+  for (int a = 0; a < 3; ++a) { U[CEX + a] = sg * E[a]; U[CBX + a] = sg * B[a]; }   // Eq. 28
+  U[CPSI] = sg * X[11]; U[CPHI] = sg * X[12]; U[CQ] = sg * X[13];
+  Gf[CD] = v[0] * U[CD];
+  const double hv = hW2 * v[0];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    double t = hv * vD[a] - E[0] * ED[a] - B[0] * BD[a];
+    if (a == 0) t += p + pem;
+    Gf[CSX + a] = sg * t;
+  }
+  Gf[CTAU] = (m.gi0[0] * U[CSX] + m.gi0[1] * U[CSX + 1] + m.gi0[2] * U[CSX + 2]) - v[0] * U[CD];
+  Gf[CBX] = m.gi0[0] * U[CPHI];
+  Gf[CBX + 1] = m.gi0[1] * U[CPHI] - ED[2];
+  Gf[CBX + 2] = m.gi0[2] * U[CPHI] + ED[1];
+  Gf[CEX] = m.gi0[0] * U[CPSI];
+  Gf[CEX + 1] = m.gi0[1] * U[CPSI] + BD[2];
+  Gf[CEX + 2] = m.gi0[2] * U[CPSI] - BD[1];
+  Gf[CPHI] = U[CBX];
+  Gf[CPSI] = U[CEX];
+  double Jc;
+  if (CHARGE == CHARGE_FACE_OHM) {   // Eq. 29 densitised: sg (v x B)^0 = v_1 B_2 - v_2 B_1
+    const double vE = E[0] * vD[0] + E[1] * vD[1] + E[2] * vD[2];
+    Jc = W * sigma * (U[CEX] + (vD[1] * BD[2] - vD[2] * BD[1]) - vE * sg * v[0]);
+  } else {
+    Jc = sg * X[14];
+  }
+  Gf[CQ] = U[CQ] * v[0] + Jc;
+#pragma unroll
+  for (int c = 0; c < NCONS; ++c) {
+    const double t = wa * Gf[c] + wu * U[c];
+    Fh[c] = FIRST ? t : Fh[c] + t;
+  }
+}
+
+// a2 for one cell along one direction, all variables: lower-face values stay in lo[] (registers);
+// upper-face / lower-face values are stored (strided) where the caller says.
+template <int RECON, int NV>
+__device__ __forceinline__ void recon_all(const PencilTabs& T, int K, long long ct, long long s, double eps_w,
+                                          double lo[NVR], double* __restrict__ hi_dst, int hi_stride, bool st_hi,
+                                          double* __restrict__ hi2_dst, bool st_hi2,
+                                          double* __restrict__ lo_dst, bool st_lo) {
+#pragma unroll
+  for (int vr = 0; vr < NV; ++vr) {
+    const double* __restrict__ f = T.P[K][vr] + ct;
+    double l, h;
+    const double um1 = f[-s], u0 = f[0], up1 = f[s];
+    if (RECON == RECON_WENO5) {
+      recon_cell<RECON>(eps_w, f[-2 * s], um1, u0, up1, f[2 * s], l, h);
+    } else {
+      recon_cell<RECON>(0.0, 0.0, um1, u0, up1, 0.0, l, h);
+    }
+    if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
+      if (!(l > 0.0)) l = u0;
+      if (!(h > 0.0)) h = u0;
+    }
+    lo[vr] = l;
+    if (st_hi) hi_dst[vr * hi_stride] = h;
+    if (st_hi2) hi2_dst[vr * TX] = h;
+    if (st_lo) lo_dst[vr * TX] = l;
+  }
+}
+
+// FACE_OHM only (reading R6): conductivity of a CELL from its primitives and metric
+__device__ __forceinline__ double sigma_cell(const GridView& G, long long c) {
+  if (G.sigma_model == SIGMA_UNIFORM) return G.sigma0;
+  if (G.sigma_model == SIGMA_ARRAY) return __ldg(G.sigma + c);
+  Met mc;
+  load_met_cell(G, c, mc);
+  double vU[3] = {G.P[VX][c], G.P[VY][c], G.P[VZ][c]}, vD[3];
+  lower(mc, vU, vD);
+  return sigma_of(G, G.P[RHO][c] * (1.0 / sqrt(1.0 - dot3(vU, vD))), c);
+}
+
+// a3 for one face: right state PR (registers), left state read from plp (strided); F in the rotated order
+template <int CHARGE, int NV>
+__device__ __forceinline__ void riemann(const GridView& G, const PencilTabs& T, int K, long long cl, long long cr,
+                                        const double* __restrict__ plp, int pl_stride, double PR[NVR], double Fh[NCONS]) {
+  FaceMet m;
+  load_face_met(T, K, cl, cr, m);
+  // HLLE weights (Eq. 30; reading R6)
+  const double c = m.alpha * sqrt(m.gi0[0]);
+  const double lp = fmax(0.0, c - m.b0), lm = fmin(0.0, -c - m.b0);
+  const double inv = 1.0 / (lp - lm);
+  const double wL = lp * inv, wR = -lm * inv, sd = lp * lm * inv;
+  double sigL = 0.0, sigR = 0.0;
+  if (CHARGE == CHARGE_FACE_OHM) { sigL = sigma_cell(G, cl); sigR = sigma_cell(G, cr); }
+  if (NV < NVR) PR[NVR - 1] = 0.0;
+  half_flux<CHARGE, true>(m, G.Gamma, PR, sigR, wR * m.alpha, sd - wR * m.b0, Fh);
+  double PL[NVR];
+#pragma unroll
+  for (int vr = 0; vr < NV; ++vr) PL[vr] = plp[vr * pl_stride];
+  if (NV < NVR) PL[NVR - 1] = 0.0;
+  half_flux<CHARGE, false>(m, G.Gamma, PL, sigL, wL * m.alpha, -sd - wL * m.b0, Fh);
+}
+}  // namespace
+
+template <int RECON, int CHARGE, int STAGE>
+__global__ void __launch_bounds__(NT, 2)
+k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilTabs T, double dt, int CZ) {
+  constexpr int NV = (CHARGE == CHARGE_CELL_CURRENT) ? NVR : NVR - 1;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem& S = *reinterpret_cast<Smem*>(smem_raw);
+  const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  const int txn = min(TX, G.n[0] - i0), tyn = min(TY, G.n[1] - j0);   // valid extent of this tile
+  const bool in = tx < txn && ty < tyn;
+  const int k0 = blockIdx.z * CZ, k1 = min(k0 + CZ, G.n[2]);
+  const long long sz = G.stride[2];
+  const int base = ty * EXW + tx;                                     // own flux slot = slot of the left state
+  long long c = cell_index(G, i0 + tx, j0 + ty, k0 - 2);
+  double dU[NCONS];
+#pragma unroll
+  for (int v = 0; v < NCONS; ++v) dU[v] = 0.0;
+  int cur = 0;
+  // k = k0-2: upper-face z states of plane k0-1; k = k0-1: z flux through the lower face of plane k0
+  for (int k = k0 - 2; k < k1; ++k, c += sz) {
+    const bool lead = k < k0;
+#pragma unroll 1
+    for (int K = lead ? 2 : 0; K < 3; ++K) {
+      const long long s = G.stride[K];
+      const int up = (K == 0) ? 1 : (K == 1) ? EXW : 0;                // own upper-face slot relative to base
+      double lo[NVR];
+      // ---- a2: reconstruction passes (p = 0: halo cells of the tile, designated lanes; p = 1: own cell)
+      {
+        bool ex_valid = false, ex_upper = false;
+        int ex_r = 0;
+        long long ex_cell = 0;
+        if (K == 0 && ty == TY - 1 && tx < 2 * TY) {                   // x: rows r, lower (-1, r) / upper (txn, r)
+          ex_r = tx & (TY - 1); ex_upper = tx >= TY; ex_valid = ex_r < tyn;
+          ex_cell = c + (long long)((ex_upper ? txn : -1) - tx) + G.stride[1] * (long long)(ex_r - ty);
+        } else if (K == 1 && ty < 2) {                                 // y: columns tx, lower (tx, -1) / upper (tx, tyn)
+          ex_r = tx; ex_upper = ty == 1; ex_valid = tx < txn;
+          ex_cell = c + G.stride[1] * (long long)((ex_upper ? tyn : -1) - ty);
+        }
+#pragma unroll 1
+        for (int p = ex_valid ? 0 : 1; p < 2; ++p) {
+          if (p == 0) {
+            double* hd = (K == 0) ? &S.ex[0][ex_r * EXW] : &S.ex[0][ex_r];
+            recon_all<RECON, NV>(T, K, ex_cell, s, G.weno_eps, lo, hd, EXP, !ex_upper, nullptr, false,
+                                 &S.exlo[0][ex_r], ex_upper);
+          } else if (in) {
+            if (K == 2) {
+              recon_all<RECON, NV>(T, K, c + sz, s, G.weno_eps, lo, &S.chi[cur ^ 1][0][tid], NT, true, nullptr, false,
+                                   nullptr, false);
+            } else {
+              const bool edge = (K == 0) ? (tx == txn - 1) : (ty == tyn - 1);
+              recon_all<RECON, NV>(T, K, c, s, G.weno_eps, lo, &S.ex[0][base + up], EXP, true,
+                                   &S.exhi[0][(K == 0) ? ty : tx], edge, nullptr, false);
+            }
+          }
+        }
+      }
+      if (K < 2) __syncthreads();                                      // A: upper-face states visible
+      // ---- a3: Riemann passes (p = 0: own lower face (x, y) / upper face (z); p = 1: faces on the tile's upper edge)
+      double F[NCONS];
+      if (K == 2) {
+        if (in && k >= k0 - 1) {
+          riemann<CHARGE, NV>(G, T, K, c, c + sz, &S.chi[cur][0][tid], NT, lo, F);
+#pragma unroll
+          for (int v = 0; v < NCONS; ++v) S.chi[cur][T.nat[K][v]][tid] = F[v];   // thread-private: the left state is consumed
+        }
+      } else {
+        bool e_valid = false;
+        int e_r = 0;
+        if (K == 0 && ty == 2 && tx < tyn) { e_valid = true; e_r = tx; }
+        if (K == 1 && ty == 3 && tx < txn) { e_valid = true; e_r = tx; }
+#pragma unroll 1
+        for (int p = 0; p < 2; ++p) {
+          bool valid;
+          long long cr;
+          const double* plp;
+          int pls, dst;
+          if (p == 0) {
+            valid = in; cr = c; plp = &S.ex[0][base]; pls = EXP; dst = base;
+          } else {
+            valid = e_valid; plp = &S.exhi[0][e_r]; pls = TX;
+            if (K == 0) { cr = c + (long long)(txn - tx) + G.stride[1] * (long long)(e_r - ty); dst = e_r * EXW + txn; }
+            else        { cr = c + G.stride[1] * (long long)(tyn - ty); dst = tyn * EXW + e_r; }
+            if (valid) {
+#pragma unroll
+              for (int vr = 0; vr < NV; ++vr) lo[vr] = S.exlo[vr][e_r];
+            }
+          }
+          if (valid) riemann<CHARGE, NV>(G, T, K, cr - s, cr, plp, pls, lo, F);
+          if (p == 0) __syncthreads();                                 // B: every left state has been read
+          if (valid) {
+#pragma unroll
+            for (int v = 0; v < NCONS; ++v) S.ex[T.nat[K][v]][dst] = F[v];
+          }
+        }
+        __syncthreads();                                               // C: fluxes visible
+        if (in) {
+          const double idx = G.inv_dx[K];
+#pragma unroll
+          for (int v = 0; v < NCONS; ++v) dU[v] -= (S.ex[v][base + up] - S.ex[v][base]) * idx;
+        }
+        __syncthreads();                                               // D: flux buffer free again
+      }
+    }
+    if (in && k >= k0 - 1) {
+      double Fz[NCONS];
+#pragma unroll
+      for (int v = 0; v < NCONS; ++v) Fz[v] = S.chi[cur][v][tid] * G.inv_dx[2];
+      if (k >= k0) {
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) dU[v] -= Fz[v];
+        // ---- a4 + a5
+        double P[NPRIM];
+#pragma unroll
+        for (int v = 0; v < NPRIM; ++v) P[v] = G.P[v][c];
+        add_sources(G, c, P, dU);
+        Met m;
+#pragma unroll
+        for (int q = 0; q < 6; ++q) m.g[q] = __ldg(G.met[MGXX + q] + c);
+        met_finish(m);
+        const double sgE[3] = {m.sg * P[EX], m.sg * P[EY], m.sg * P[EZ]};
+        stage_combine<STAGE>(G, c, dt, dU, sgE);
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) Fz[v] = S.chi[cur][v][tid] * G.inv_dx[2];
+      }
+#pragma unroll
+      for (int v = 0; v < NCONS; ++v) dU[v] = Fz[v];                   // lower z face of the next plane
+    }
+    cur ^= 1;
+  }
+}
+
+bool rhs_pencil_supported(const GridView& G) {
+  return G.n[0] > 1 && G.n[1] > 1 && G.n[2] > 1;
+}
+
+static int choose_cz(const GridView& G) {
+  // several waves of 148 SMs x 2 CTAs, but long enough pencils to amortise the two lead-in planes
+  const long long tiles = (long long)((G.n[0] + TX - 1) / TX) * ((G.n[1] + TY - 1) / TY);
+  int cz = 64;
+  while (cz > 8 && tiles * ((G.n[2] + cz - 1) / cz) < 148LL * 2 * 4) cz /= 2;
+  return cz;
+}
+
+static PencilTabs make_tabs(const GridView& G) {
+  PencilTabs T;
+  for (int K = 0; K < 3; ++K) {
+    const int r[3] = {K, (K + 1) % 3, (K + 2) % 3};
+    T.P[K][0] = G.P[RHO]; T.P[K][1] = G.P[PRS];
+    for (int a = 0; a < 3; ++a) {
+      T.P[K][2 + a] = G.P[VX + r[a]];
+      T.P[K][5 + a] = G.P[EX + r[a]];
+      T.P[K][8 + a] = G.P[BX + r[a]];
+    }
+    T.P[K][11] = G.P[PSI]; T.P[K][12] = G.P[PHI]; T.P[K][13] = G.P[QCH];
+    T.P[K][14] = G.jc[K];
+    T.M[K][0] = G.met[MALP];
+    T.M[K][1] = G.met[MBX + K];
+    static const int symtab[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};   // xx xy xz yy yz zz
+    int q = 0;
+    for (int a = 0; a < 3; ++a)
+      for (int b = a; b < 3; ++b) T.M[K][2 + q++] = G.met[MGXX + symtab[r[a]][r[b]]];
+    for (int v = 0; v < NCONS; ++v) T.nat[K][v] = v;
+    for (int a = 0; a < 3; ++a) {
+      T.nat[K][CSX + a] = CSX + r[a];
+      T.nat[K][CEX + a] = CEX + r[a];
+      T.nat[K][CBX + a] = CBX + r[a];
+    }
+  }
+  return T;
+}
+
+template <int RECON, int CHARGE, int STAGE>
+static cudaError_t launch_one(const GridView& G, double dt, cudaStream_t st) {
+  const int cz = choose_cz(G);
+  const PencilTabs T = make_tabs(G);
+  dim3 block(TX, TY, 1);
+  dim3 grid((G.n[0] + TX - 1) / TX, (G.n[1] + TY - 1) / TY, (G.n[2] + cz - 1) / cz);
+  const size_t smem = sizeof(Smem);
+  cudaError_t e = cudaFuncSetAttribute(k_rhs_pencil<RECON, CHARGE, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_rhs_pencil<RECON, CHARGE, STAGE><<<grid, block, smem, st>>>(G, T, dt, cz);
+  return cudaGetLastError();
+}
+
+template <int RECON, int CHARGE>
+static cudaError_t launch_rc(const GridView& G, double dt, int stage, cudaStream_t st) {
+  return stage == 1 ? launch_one<RECON, CHARGE, 1>(G, dt, st) : launch_one<RECON, CHARGE, 2>(G, dt, st);
+}
+
+cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, cudaStream_t st) {
+  const bool ohm = G.charge_mode == CHARGE_FACE_OHM;
+  switch (recon) {
+    case RECON_MINMOD:
+      return ohm ? launch_rc<RECON_MINMOD, CHARGE_FACE_OHM>(G, dt, stage, st)
+                 : launch_rc<RECON_MINMOD, CHARGE_CELL_CURRENT>(G, dt, stage, st);
+    case RECON_MC:
+      return ohm ? launch_rc<RECON_MC, CHARGE_FACE_OHM>(G, dt, stage, st)
+                 : launch_rc<RECON_MC, CHARGE_CELL_CURRENT>(G, dt, stage, st);
+    default:
+      return ohm ? launch_rc<RECON_WENO5, CHARGE_FACE_OHM>(G, dt, stage, st)
+                 : launch_rc<RECON_WENO5, CHARGE_CELL_CURRENT>(G, dt, stage, st);
+  }
+}
+
+}  // namespace rg
