@@ -67,98 +67,100 @@ __device__ __forceinline__ double d4(const double* __restrict__ f, long long c, 
 
 // a4 (second half). explicit sources at a cell centre (Eq. 27 S; Eq. 39-40;
 // reading R1 / SURVEY.md O6).  P = the cell's primitives; ADDS the sources to S[].
+//   S(S_i)  = 1/2 alpha sg T^jk d_i gamma_jk + S_j d_i beta^j - (tau + D) d_i alpha
+//   S(tau)  = alpha sg T^ij K_ij - S^j d_j alpha
+//   S(calB^i) = -calB^k d_k beta^i + Phi G^i ;  S(calE^i) = -calE^k d_k beta^i + Psi G^i - alpha calQ v^i
+//   S(Phi)  = -alpha Phi K + calB^k d_k alpha - alpha kappa Phi ;  S(Psi) likewise + alpha calQ
+//   G^i = gamma^ij d_j alpha - alpha gamma^il gamma^jk (d_j gamma_lk - 1/2 d_l gamma_jk)
+// The metric derivatives (4th-order centred, reading R2) are consumed direction by direction so that
+// only one direction's ten derivatives are live at a time.
 __device__ __forceinline__ void add_sources(const GridView& G, long long c, const double P[NPRIM], double S[NCONS]) {
   Met m;
   load_met_cell(G, c, m);
-  double KDD[6];
-#pragma unroll
-  for (int q = 0; q < 6; ++q) KDD[q] = __ldg(G.met[MKXX + q] + c);
-  double dalpha[3], dbeta[3][3], dg[3][6];   // dalpha[k] = d_k alpha; dbeta[k][i] = d_k beta^i; dg[k][q] = d_k gamma_q
-#pragma unroll
-  for (int kk = 0; kk < 3; ++kk) {
-    if (G.n[kk] > 1) {
-      const long long s = G.stride[kk];
-      const double w = G.inv_12dx[kk];
-      dalpha[kk] = d4(G.met[MALP], c, s, w);
-#pragma unroll
-      for (int a = 0; a < 3; ++a) dbeta[kk][a] = d4(G.met[MBX + a], c, s, w);
-#pragma unroll
-      for (int q = 0; q < 6; ++q) dg[kk][q] = d4(G.met[MGXX + q], c, s, w);
-    } else {
-      dalpha[kk] = 0.0;
-#pragma unroll
-      for (int a = 0; a < 3; ++a) dbeta[kk][a] = 0.0;
-#pragma unroll
-      for (int q = 0; q < 6; ++q) dg[kk][q] = 0.0;
-    }
-  }
-  double U[NCONS];
-  prim2cons(m, G.Gamma, P, U);
   const double rho = P[RHO], p = P[PRS];
   const double vU[3] = {P[VX], P[VY], P[VZ]}, EU[3] = {P[EX], P[EY], P[EZ]}, BU[3] = {P[BX], P[BY], P[BZ]};
-  double vD[3], ED[3], BD[3];
+  double vD[3], ED[3], BD[3], ExB[3];
   lower(m, vU, vD); lower(m, EU, ED); lower(m, BU, BD);
+  cross_raw(EU, BU, ExB);
   const double v2 = dot3(vU, vD), W2 = 1.0 / (1.0 - v2);
   const double h = rho + G.Gamma / (G.Gamma - 1.0) * p;
   const double pem = 0.5 * (dot3(EU, ED) + dot3(BU, BD)), hW2 = h * W2;
-  // T^ab = h W^2 v^a v^b + g^ab (p + (E^2+B^2)/2) - E^a E^b - B^a B^b   (symmetric storage)
-  double T[6];
+  const double al = m.alpha, sg = m.sg;
+  // T^ab = h W^2 v^a v^b + g^ab (p + (E^2+B^2)/2) - E^a E^b - B^a B^b, stored with the symmetric-contraction
+  // weights (1,2,2,1,2,1) folded in:  X^ab Y_ab = sum_q Tw_q Y_q
+  double Tw[6];
 #pragma unroll
   for (int a = 0; a < 3; ++a)
 #pragma unroll
-    for (int b = a; b < 3; ++b)
-      T[sym(a, b)] = hW2 * vU[a] * vU[b] + m.gi[sym(a, b)] * (p + pem) - EU[a] * EU[b] - BU[a] * BU[b];
-  const double al = m.alpha, sg = m.sg;
-  const double SD[3] = {U[CSX], U[CSY], U[CSZ]};
+    for (int b = a; b < 3; ++b) {
+      const double t = hW2 * vU[a] * vU[b] + m.gi[sym(a, b)] * (p + pem) - EU[a] * EU[b] - BU[a] * BU[b];
+      Tw[sym(a, b)] = (a == b) ? t : 2.0 * t;
+    }
+  double SD[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) SD[a] = sg * (hW2 * vD[a] + sg * ExB[a]);            // Eq. 24
   double SU[3];
   raise(m, SD, SU);
-  // symmetric contraction X^ab Y_ab = sum_q w_q X_q Y_q, w = (1,2,2,1,2,1)
-  const double wq[6] = {1.0, 2.0, 2.0, 1.0, 2.0, 1.0};
+  const double tauD = sg * (hW2 - p + pem);                                         // tau + D (Eq. 22-23)
+  const double cE[3] = {sg * EU[0], sg * EU[1], sg * EU[2]}, cB[3] = {sg * BU[0], sg * BU[1], sg * BU[2]};
+  const double cPsi = sg * P[PSI], cPhi = sg * P[PHI], cQ = sg * P[QCH];
+  const double asg = al * sg;
+  double trK = 0.0;
+  {
+    double t1 = 0.0;
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+      const double Kq = __ldg(G.met[MKXX + q] + c);
+      t1 += Tw[q] * Kq;
+      trK += ((q == 0 || q == 3 || q == 5) ? 1.0 : 2.0) * m.gi[q] * Kq;
+    }
+    S[CTAU] += asg * t1;
+  }
+  double Cl[3] = {0.0, 0.0, 0.0}, da[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    if (G.n[d] > 1) {
+      const long long s = G.stride[d];
+      const double w = G.inv_12dx[d];
+      const double dal = d4(G.met[MALP], c, s, w);
+      double db[3], dg[6];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) db[a] = d4(G.met[MBX + a], c, s, w);
+#pragma unroll
+      for (int q = 0; q < 6; ++q) dg[q] = d4(G.met[MGXX + q], c, s, w);
+      da[d] = dal;
+      double tg = 0.0, gdg = 0.0;
+#pragma unroll
+      for (int q = 0; q < 6; ++q) {
+        tg += Tw[q] * dg[q];
+        gdg += ((q == 0 || q == 3 || q == 5) ? 1.0 : 2.0) * m.gi[q] * dg[q];
+      }
+      S[CSX + d] += 0.5 * asg * tg + (SD[0] * db[0] + SD[1] * db[1] + SD[2] * db[2]) - tauD * dal;
+      S[CTAU] -= SU[d] * dal;
+#pragma unroll
+      for (int l = 0; l < 3; ++l)
+        Cl[l] += m.gi[sym(d, 0)] * dg[sym(l, 0)] + m.gi[sym(d, 1)] * dg[sym(l, 1)] + m.gi[sym(d, 2)] * dg[sym(l, 2)];
+      Cl[d] -= 0.5 * gdg;
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        S[CBX + a] -= cB[d] * db[a];
+        S[CEX + a] -= cE[d] * db[a];
+      }
+      S[CPHI] += cB[d] * dal;
+      S[CPSI] += cE[d] * dal;
+    }
+  }
+  double Gi[3], gda[3];
+  raise(m, Cl, Gi);
+  raise(m, da, gda);
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    double t1 = 0.0, t2 = 0.0;
-#pragma unroll
-    for (int q = 0; q < 6; ++q) t1 += wq[q] * T[q] * dg[a][q];
-#pragma unroll
-    for (int b = 0; b < 3; ++b) t2 += SD[b] * dbeta[a][b];
-    S[CSX + a] += 0.5 * al * sg * t1 + t2 - (U[CTAU] + U[CD]) * dalpha[a];
+    const double Ga = gda[a] - al * Gi[a];
+    S[CBX + a] += cPhi * Ga;
+    S[CEX + a] += cPsi * Ga - al * cQ * vU[a];
   }
-  {
-    double t1 = 0.0, trK = 0.0;
-#pragma unroll
-    for (int q = 0; q < 6; ++q) { t1 += wq[q] * T[q] * KDD[q]; trK += wq[q] * m.gi[q] * KDD[q]; }
-    S[CTAU] += al * sg * t1 - dot3(SU, dalpha);
-    // G^i = gamma^ij d_j alpha - alpha gamma^il gamma^jk (d_j gamma_lk - 1/2 d_l gamma_jk)
-    double Cl[3];
-#pragma unroll
-    for (int l = 0; l < 3; ++l) {
-      double t = 0.0;
-#pragma unroll
-      for (int j = 0; j < 3; ++j)
-#pragma unroll
-        for (int k2 = 0; k2 < 3; ++k2)
-          t += m.gi[sym(j, k2)] * (dg[j][sym(l, k2)] - 0.5 * dg[l][sym(j, k2)]);
-      Cl[l] = t;
-    }
-    double Gi[3], gda[3];
-    raise(m, Cl, Gi);
-    raise(m, dalpha, gda);
-#pragma unroll
-    for (int a = 0; a < 3; ++a) Gi[a] = gda[a] - al * Gi[a];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      double tB = 0.0, tE = 0.0;
-#pragma unroll
-      for (int kk = 0; kk < 3; ++kk) { tB += U[CBX + kk] * dbeta[kk][a]; tE += U[CEX + kk] * dbeta[kk][a]; }
-      S[CBX + a] += -tB + U[CPHI] * Gi[a];
-      S[CEX + a] += -tE + U[CPSI] * Gi[a] - al * U[CQ] * vU[a];
-    }
-    double BdA = 0.0, EdA = 0.0;
-#pragma unroll
-    for (int kk = 0; kk < 3; ++kk) { BdA += U[CBX + kk] * dalpha[kk]; EdA += U[CEX + kk] * dalpha[kk]; }
-    S[CPHI] += -al * U[CPHI] * trK + BdA - al * G.kappa * U[CPHI];
-    S[CPSI] += -al * U[CPSI] * trK + EdA + al * U[CQ] - al * G.kappa * U[CPSI];
-  }
+  S[CPHI] -= al * cPhi * (trK + G.kappa);
+  S[CPSI] += al * (cQ - cPsi * (trK + G.kappa));
 }
 
 // a5. IMEX-SSP2(2,2,2) stage combine (Eq. 35-37; gamma = 1 - 1/sqrt(2); readings R11, R12)

@@ -39,7 +39,8 @@ struct Smem {
   double ex[NVR][EXP];       // upper-face states of the tile's cells (+ lower halo); later the face fluxes
   double exlo[NVR][TX];      // lower-face states of the upper-halo cells
   double exhi[NVR][TX];      // upper-face states of the last interior row/column (left states of the edge faces)
-  double chi[2][NVR][NT];    // z: upper-face states of the current plane (ping-pong), then the z flux
+  double chi[NVR][NT];       // z carry: upper-face states of the current plane (left states of its upper z faces)
+  double du[NCONS][NT];      // flux divergence being accumulated for the current plane (thread-private slots)
 };
 
 struct FaceMet {
@@ -206,13 +207,9 @@ k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilT
   const int txn = min(TX, G.n[0] - i0), tyn = min(TY, G.n[1] - j0);   // valid extent of this tile
   const bool in = tx < txn && ty < tyn;
   const int k0 = blockIdx.z * CZ, k1 = min(k0 + CZ, G.n[2]);
-  const long long sz = G.stride[2];
+  const long long sy = G.stride[1], sz = G.stride[2];
   const int base = ty * EXW + tx;                                     // own flux slot = slot of the left state
   long long c = cell_index(G, i0 + tx, j0 + ty, k0 - 2);
-  double dU[NCONS];
-#pragma unroll
-  for (int v = 0; v < NCONS; ++v) dU[v] = 0.0;
-  int cur = 0;
   // k = k0-2: upper-face z states of plane k0-1; k = k0-1: z flux through the lower face of plane k0
   for (int k = k0 - 2; k < k1; ++k, c += sz) {
     const bool lead = k < k0;
@@ -220,6 +217,7 @@ k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilT
     for (int K = lead ? 2 : 0; K < 3; ++K) {
       const long long s = G.stride[K];
       const int up = (K == 0) ? 1 : (K == 1) ? EXW : 0;                // own upper-face slot relative to base
+      const long long cm = (K == 2) ? c + sz : c;                      // the cell this thread reconstructs
       double lo[NVR];
       // ---- a2: reconstruction passes (p = 0: halo cells of the tile, designated lanes; p = 1: own cell)
       {
@@ -228,39 +226,33 @@ k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilT
         long long ex_cell = 0;
         if (K == 0 && ty == TY - 1 && tx < 2 * TY) {                   // x: rows r, lower (-1, r) / upper (txn, r)
           ex_r = tx & (TY - 1); ex_upper = tx >= TY; ex_valid = ex_r < tyn;
-          ex_cell = c + (long long)((ex_upper ? txn : -1) - tx) + G.stride[1] * (long long)(ex_r - ty);
+          ex_cell = c + (long long)((ex_upper ? txn : -1) - tx) + sy * (long long)(ex_r - ty);
         } else if (K == 1 && ty < 2) {                                 // y: columns tx, lower (tx, -1) / upper (tx, tyn)
           ex_r = tx; ex_upper = ty == 1; ex_valid = tx < txn;
-          ex_cell = c + G.stride[1] * (long long)((ex_upper ? tyn : -1) - ty);
+          ex_cell = c + sy * (long long)((ex_upper ? tyn : -1) - ty);
         }
 #pragma unroll 1
         for (int p = ex_valid ? 0 : 1; p < 2; ++p) {
+          long long ct;
+          double *hd, *h2, *ld;
+          bool sth, sth2, stl, valid;
           if (p == 0) {
-            double* hd = (K == 0) ? &S.ex[0][ex_r * EXW] : &S.ex[0][ex_r];
-            recon_all<RECON, NV>(T, K, ex_cell, s, G.weno_eps, lo, hd, EXP, !ex_upper, nullptr, false,
-                                 &S.exlo[0][ex_r], ex_upper);
-          } else if (in) {
-            if (K == 2) {
-              recon_all<RECON, NV>(T, K, c + sz, s, G.weno_eps, lo, &S.chi[cur ^ 1][0][tid], NT, true, nullptr, false,
-                                   nullptr, false);
-            } else {
-              const bool edge = (K == 0) ? (tx == txn - 1) : (ty == tyn - 1);
-              recon_all<RECON, NV>(T, K, c, s, G.weno_eps, lo, &S.ex[0][base + up], EXP, true,
-                                   &S.exhi[0][(K == 0) ? ty : tx], edge, nullptr, false);
-            }
+            ct = ex_cell; valid = true;
+            hd = (K == 0) ? &S.ex[0][ex_r * EXW] : &S.ex[0][ex_r]; sth = !ex_upper;
+            h2 = hd; sth2 = false;
+            ld = &S.exlo[0][ex_r]; stl = ex_upper;
+          } else {
+            ct = cm; valid = in;
+            hd = &S.ex[0][base + up]; sth = true;
+            h2 = &S.exhi[0][(K == 0) ? ty : tx]; sth2 = (K == 0) ? (tx == txn - 1) : (K == 1) ? (ty == tyn - 1) : false;
+            ld = hd; stl = false;
           }
+          if (valid) recon_all<RECON, NV>(T, K, ct, s, G.weno_eps, lo, hd, EXP, sth, h2, sth2, ld, stl);
         }
       }
       if (K < 2) __syncthreads();                                      // A: upper-face states visible
       // ---- a3: Riemann passes (p = 0: own lower face (x, y) / upper face (z); p = 1: faces on the tile's upper edge)
-      double F[NCONS];
-      if (K == 2) {
-        if (in && k >= k0 - 1) {
-          riemann<CHARGE, NV>(G, T, K, c, c + sz, &S.chi[cur][0][tid], NT, lo, F);
-#pragma unroll
-          for (int v = 0; v < NCONS; ++v) S.chi[cur][T.nat[K][v]][tid] = F[v];   // thread-private: the left state is consumed
-        }
-      } else {
+      {
         bool e_valid = false;
         int e_r = 0;
         if (K == 0 && ty == 2 && tx < tyn) { e_valid = true; e_r = tx; }
@@ -272,39 +264,51 @@ k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilT
           const double* plp;
           int pls, dst;
           if (p == 0) {
-            valid = in; cr = c; plp = &S.ex[0][base]; pls = EXP; dst = base;
+            valid = in && k >= k0 - 1; cr = cm; dst = base;
+            plp = (K == 2) ? &S.chi[0][tid] : &S.ex[0][base];
+            pls = (K == 2) ? NT : EXP;
           } else {
             valid = e_valid; plp = &S.exhi[0][e_r]; pls = TX;
-            if (K == 0) { cr = c + (long long)(txn - tx) + G.stride[1] * (long long)(e_r - ty); dst = e_r * EXW + txn; }
-            else        { cr = c + G.stride[1] * (long long)(tyn - ty); dst = tyn * EXW + e_r; }
+            if (K == 0) { cr = c + (long long)(txn - tx) + sy * (long long)(e_r - ty); dst = e_r * EXW + txn; }
+            else        { cr = c + sy * (long long)(tyn - ty); dst = tyn * EXW + e_r; }
             if (valid) {
 #pragma unroll
               for (int vr = 0; vr < NV; ++vr) lo[vr] = S.exlo[vr][e_r];
             }
           }
+          double F[NCONS];
           if (valid) riemann<CHARGE, NV>(G, T, K, cr - s, cr, plp, pls, lo, F);
-          if (p == 0) __syncthreads();                                 // B: every left state has been read
+          if (p == 0) {
+            if (K < 2) __syncthreads();                                // B: every left state has been read
+            else if (in) {                                             // z: the new upper-face states become the carry
+#pragma unroll
+              for (int vr = 0; vr < NV; ++vr) S.chi[vr][tid] = S.ex[vr][base];
+            }
+          }
           if (valid) {
 #pragma unroll
             for (int v = 0; v < NCONS; ++v) S.ex[T.nat[K][v]][dst] = F[v];
           }
         }
+      }
+      if (K < 2) {
         __syncthreads();                                               // C: fluxes visible
         if (in) {
           const double idx = G.inv_dx[K];
 #pragma unroll
-          for (int v = 0; v < NCONS; ++v) dU[v] -= (S.ex[v][base + up] - S.ex[v][base]) * idx;
+          for (int v = 0; v < NCONS; ++v) S.du[v][tid] -= (S.ex[v][base + up] - S.ex[v][base]) * idx;
         }
-        __syncthreads();                                               // D: flux buffer free again
       }
     }
     if (in && k >= k0 - 1) {
-      double Fz[NCONS];
+      double dU[NCONS];
 #pragma unroll
-      for (int v = 0; v < NCONS; ++v) Fz[v] = S.chi[cur][v][tid] * G.inv_dx[2];
+      for (int v = 0; v < NCONS; ++v) {
+        const double Fz = S.ex[v][base] * G.inv_dx[2];
+        dU[v] = S.du[v][tid] - Fz;
+        S.du[v][tid] = Fz;                                             // lower z face of the next plane
+      }
       if (k >= k0) {
-#pragma unroll
-        for (int v = 0; v < NCONS; ++v) dU[v] -= Fz[v];
         // ---- a4 + a5
         double P[NPRIM];
 #pragma unroll
@@ -316,13 +320,9 @@ k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilT
         met_finish(m);
         const double sgE[3] = {m.sg * P[EX], m.sg * P[EY], m.sg * P[EZ]};
         stage_combine<STAGE>(G, c, dt, dU, sgE);
-#pragma unroll
-        for (int v = 0; v < NCONS; ++v) Fz[v] = S.chi[cur][v][tid] * G.inv_dx[2];
       }
-#pragma unroll
-      for (int v = 0; v < NCONS; ++v) dU[v] = Fz[v];                   // lower z face of the next plane
     }
-    cur ^= 1;
+    __syncthreads();                                                   // D: exchange buffer free for the next plane
   }
 }
 
