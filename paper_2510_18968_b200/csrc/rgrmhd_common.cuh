@@ -65,6 +65,42 @@ __device__ __forceinline__ constexpr int sym(int i, int j) {
   return (i == 0) ? j : (j == 0) ? i : (i == 1) ? ((j == 1) ? 3 : 4) : ((j == 1) ? 4 : 5);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Branch-free FP64 reciprocal / square root: hardware seed (MUFU.RCP64H / MUFU.RSQ64H, >= 20 good
+// bits) + Newton steps in DFMA.  Result within ~1 ulp of the correctly rounded value for normal,
+// positive-finite arguments (every use below: determinants, 1 - v^2, WENO weight sums); no special-case
+// path, so the surrounding code stays one basic block and independent chains interleave.  The
+// difference to IEEE division is a rounding-level one.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double rcp_fast(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+// g = sqrt(x), rs = 1/sqrt(x) (coupled Newton iteration on g ~ sqrt(x), h ~ 1/(2 sqrt(x)))
+__device__ __forceinline__ void sqrt_rsqrt_fast(double x, double& g, double& rs) {
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  g = x * r;
+  double h = 0.5 * r;
+  double e = fma(-g, h, 0.5);
+  g = fma(g, e, g); h = fma(h, e, h);
+  e = fma(-g, h, 0.5);
+  g = fma(g, e, g); h = fma(h, e, h);
+  e = fma(-g, h, 0.5);
+  h = fma(h, e, h);
+  const double d = fma(-g, g, x);
+  g = fma(d, h, g);
+  rs = h + h;
+}
+__device__ __forceinline__ double sqrt_fast(double x) { double g, rs; sqrt_rsqrt_fast(x, g, rs); return g; }
+__device__ __forceinline__ double rsqrt_fast(double x) { double g, rs; sqrt_rsqrt_fast(x, g, rs); return rs; }
+
 // sqrt(gamma) and gamma^ij = adjugate/det from gamma_ij
 __device__ __forceinline__ void met_finish(Met& m) {
   const double gxx = m.g[0], gxy = m.g[1], gxz = m.g[2], gyy = m.g[3], gyz = m.g[4], gzz = m.g[5];
@@ -72,8 +108,8 @@ __device__ __forceinline__ void met_finish(Met& m) {
   const double cxy = gxz * gyz - gxy * gzz;
   const double cxz = gxy * gyz - gxz * gyy;
   const double det = gxx * cxx + gxy * cxy + gxz * cxz;
-  const double idet = 1.0 / det;
-  m.sg = sqrt(det);
+  const double idet = rcp_fast(det);
+  m.sg = sqrt_fast(det);
   m.gi[0] = cxx * idet;
   m.gi[1] = cxy * idet;
   m.gi[2] = cxz * idet;
@@ -263,16 +299,37 @@ __device__ __forceinline__ double weno5_eval(double u0, double u1, double u2, do
   const double q2 = 2.0 * u2 + 5.0 * u3 - u4;
   const double p12 = b1 * b2, p02 = b0 * b2, p01 = b0 * b1;
   const double a0 = 0.1 * (p12 * p12), a1 = 0.6 * (p02 * p02), a2 = 0.3 * (p01 * p01);
-  return (a0 * q0 + a1 * q1 + a2 * q2) / (6.0 * (a0 + a1 + a2));
+  return (a0 * q0 + a1 * q1 + a2 * q2) * rcp_fast(6.0 * (a0 + a1 + a2));
+}
+// Both face values of the centre cell u2 from one set of smoothness indicators.  Same weights as
+// weno5_eval (d_k / b_k^2 in product form, d = (0.1, 0.6, 0.3) seen from the face), candidates with the
+// 1/6 folded in; lo is the mirror image of hi.
+__device__ __forceinline__ void weno5_pair(double u0, double u1, double u2, double u3, double u4, double eps_w,
+                                           double& lo, double& hi) {
+  double b0, b1, b2;
+  weno5_beta(u0, u1, u2, u3, u4, eps_w, b0, b1, b2);
+  const double p12 = b1 * b2, p02 = b0 * b2, p01 = b0 * b1;
+  const double s12 = p12 * p12, s02 = p02 * p02, s01 = p01 * p01;
+  const double wB = 0.6 * s02;
+  const double hA = 0.1 * s12, hC = 0.3 * s01;     // hi: stencils {u0,u1,u2}, {u1,u2,u3}, {u2,u3,u4}
+  const double lA = 0.1 * s01, lC = 0.3 * s12;     // lo: stencils {u4,u3,u2}, {u3,u2,u1}, {u2,u1,u0}
+  constexpr double c13 = 1.0 / 3.0, c76 = 7.0 / 6.0, c116 = 11.0 / 6.0, c16 = 1.0 / 6.0, c56 = 5.0 / 6.0;
+  const double hq0 = fma(c13, u0, fma(-c76, u1, c116 * u2));
+  const double hq1 = fma(-c16, u1, fma(c56, u2, c13 * u3));
+  const double hq2 = fma(c13, u2, fma(c56, u3, -c16 * u4));
+  const double lq0 = fma(c13, u4, fma(-c76, u3, c116 * u2));
+  const double lq1 = fma(-c16, u3, fma(c56, u2, c13 * u1));
+  const double lq2 = fma(c13, u2, fma(c56, u1, -c16 * u0));
+  const double hn = fma(hA, hq0, fma(wB, hq1, hC * hq2)), hd = hA + wB + hC;
+  const double ln = fma(lA, lq0, fma(wB, lq1, lC * lq2)), ld = lA + wB + lC;
+  hi = hn * rcp_fast(hd);
+  lo = ln * rcp_fast(ld);
 }
 template <int RECON>
 __device__ __forceinline__ void recon_cell(double eps_w, double um2, double um1, double u0, double up1, double up2,
                                            double& lo, double& hi) {
   if (RECON == RECON_WENO5) {
-    double b0, b1, b2;
-    weno5_beta(um2, um1, u0, up1, up2, eps_w, b0, b1, b2);
-    hi = weno5_eval(um2, um1, u0, up1, up2, b0, b1, b2);
-    lo = weno5_eval(up2, up1, u0, um1, um2, b2, b1, b0);      // mirror image
+    weno5_pair(um2, um1, u0, up1, up2, eps_w, lo, hi);
   } else {
     const double a = u0 - um1, b = up1 - u0;
     const double slope = (RECON == RECON_MINMOD) ? minmod2(a, b) : minmod3(2.0 * a, 2.0 * b, 0.5 * (a + b));

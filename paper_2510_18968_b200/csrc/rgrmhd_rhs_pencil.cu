@@ -58,8 +58,8 @@ __device__ __forceinline__ void load_face_met(const PencilTabs& T, int K, long l
   const double c01 = m.g[2] * m.g[4] - m.g[1] * m.g[5];
   const double c02 = m.g[1] * m.g[4] - m.g[2] * m.g[3];
   const double det = m.g[0] * c00 + m.g[1] * c01 + m.g[2] * c02;
-  const double idet = 1.0 / det;
-  m.sg = sqrt(det);
+  const double idet = rcp_fast(det);
+  m.sg = sqrt_fast(det);
   m.gi0[0] = c00 * idet; m.gi0[1] = c01 * idet; m.gi0[2] = c02 * idet;
 }
 
@@ -79,7 +79,7 @@ __device__ __forceinline__ void half_flux(const FaceMet& m, double Gamma, const 
   double vsq = v[0] * vD[0] + v[1] * vD[1] + v[2] * vD[2];
   const double v2max = 1.0 - 1e-10;
   if (vsq >= v2max) {   // reading R4: limit |v| of a face state with the face metric
-    const double f = sqrt(v2max / vsq);
+    const double f = sqrt_fast(v2max * rcp_fast(vsq));
 #pragma unroll
     for (int a = 0; a < 3; ++a) { v[a] *= f; vD[a] *= f; }
     vsq = v[0] * vD[0] + v[1] * vD[1] + v[2] * vD[2];
@@ -88,7 +88,7 @@ __device__ __forceinline__ void half_flux(const FaceMet& m, double Gamma, const 
                         m.g[2] * E[0] + m.g[4] * E[1] + m.g[5] * E[2]};
   const double BD[3] = {m.g[0] * B[0] + m.g[1] * B[1] + m.g[2] * B[2], m.g[1] * B[0] + m.g[3] * B[1] + m.g[4] * B[2],
                         m.g[2] * B[0] + m.g[4] * B[1] + m.g[5] * B[2]};
-  const double W = 1.0 / sqrt(1.0 - vsq);
+  const double W = rsqrt_fast(1.0 - vsq);
   const double h = rho + Gamma / (Gamma - 1.0) * p;              // rho(1+eps)+p with Eq. 49
   const double hW2 = h * W * W;
   const double pem = 0.5 * ((E[0] * ED[0] + E[1] * ED[1] + E[2] * ED[2]) + (B[0] * BD[0] + B[1] * BD[1] + B[2] * BD[2]));
@@ -134,31 +134,87 @@ __device__ __forceinline__ void half_flux(const FaceMet& m, double Gamma, const 
   }
 }
 
-// a2 for one cell along one direction, all variables: lower-face values stay in lo[] (registers);
-// upper-face / lower-face values are stored (strided) where the caller says.
+// stencil of one variable along one direction (TVD uses the inner three values only)
+template <int RECON>
+__device__ __forceinline__ void load_stencil(const double* __restrict__ f, long long s, double u[5]) {
+  if (RECON == RECON_WENO5) { u[0] = f[-2 * s]; u[4] = f[2 * s]; } else { u[0] = 0.0; u[4] = 0.0; }
+  u[1] = f[-s]; u[2] = f[0]; u[3] = f[s];
+}
+
+// a2 for the thread's own cell along direction K, all variables: lower-face values stay in lo[]
+// (registers), upper-face values go to hi_dst (strided) and, for the last cell of a row / column, also
+// to hi2_dst.  The loads run PF variables ahead of the arithmetic (software pipeline in registers).
 template <int RECON, int NV>
-__device__ __forceinline__ void recon_all(const PencilTabs& T, int K, long long ct, long long s, double eps_w,
-                                          double lo[NVR], double* __restrict__ hi_dst, int hi_stride, bool st_hi,
-                                          double* __restrict__ hi2_dst, bool st_hi2,
-                                          double* __restrict__ lo_dst, bool st_lo) {
+__device__ __forceinline__ void recon_own(const PencilTabs& T, int K, long long ct, long long s, double eps_w,
+                                          double lo[NVR], double* __restrict__ hi_dst, int hi_stride,
+                                          double* __restrict__ hi2_dst, bool st_hi2) {
+  constexpr int PF = 2;
+  double buf[PF + 1][5];
+#pragma unroll
+  for (int vr = 0; vr < PF && vr < NV; ++vr) load_stencil<RECON>(T.P[K][vr] + ct, s, buf[vr]);
 #pragma unroll
   for (int vr = 0; vr < NV; ++vr) {
-    const double* __restrict__ f = T.P[K][vr] + ct;
+    if (vr + PF < NV) load_stencil<RECON>(T.P[K][vr + PF] + ct, s, buf[(vr + PF) % (PF + 1)]);
+    const double* u = buf[vr % (PF + 1)];
     double l, h;
-    const double um1 = f[-s], u0 = f[0], up1 = f[s];
-    if (RECON == RECON_WENO5) {
-      recon_cell<RECON>(eps_w, f[-2 * s], um1, u0, up1, f[2 * s], l, h);
-    } else {
-      recon_cell<RECON>(0.0, 0.0, um1, u0, up1, 0.0, l, h);
-    }
+    recon_cell<RECON>(eps_w, u[0], u[1], u[2], u[3], u[4], l, h);
     if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
-      if (!(l > 0.0)) l = u0;
-      if (!(h > 0.0)) h = u0;
+      if (!(l > 0.0)) l = u[2];
+      if (!(h > 0.0)) h = u[2];
     }
     lo[vr] = l;
-    if (st_hi) hi_dst[vr * hi_stride] = h;
+    hi_dst[vr * hi_stride] = h;
     if (st_hi2) hi2_dst[vr * TX] = h;
-    if (st_lo) lo_dst[vr * TX] = l;
+  }
+}
+
+// a2 for the halo cells of the tile (x, y only): the cell below the tile's first row / column gives the
+// left state of the tile's first faces (its upper-face value -> ex halo slot); the cell above the last
+// row / column gives the right state of the tile's edge faces (its lower-face value -> exlo).  Work
+// unit = (variable, lower | upper) x one lane per row (x: 2*TY lanes) or per column (y: TX lanes);
+// the units are dealt round-robin to the TY warps so that every warp carries the same extra load.
+template <int RECON, int NV>
+__device__ __forceinline__ void recon_halo(const PencilTabs& T, int K, Smem& S, long long c, long long s, long long sy,
+                                           double eps_w, int tx, int ty, int txn, int tyn) {
+  const int nunits = (K == 0) ? NV : 2 * NV;
+  bool upper, valid;
+  int r;
+  long long cell;
+  if (K == 0) {
+    r = tx % TY; upper = (tx / TY) == 1; valid = tx < 2 * TY && r < tyn;
+    cell = c + (long long)((upper ? txn : -1) - tx) + sy * (long long)(r - ty);
+  } else {
+    r = tx; upper = false; valid = tx < txn;
+    cell = 0;
+  }
+  double cur[5], nxt[5];
+  auto unit_ptr = [&](int u, bool& up_u) -> const double* {
+    if (K == 0) { up_u = upper; return T.P[K][u] + cell; }
+    up_u = (u & 1) != 0;
+    return T.P[K][u >> 1] + (c + sy * (long long)((up_u ? tyn : -1) - ty));
+  };
+  bool up_c = false, up_n = false;
+  int u = ty;
+  if (valid && u < nunits) load_stencil<RECON>(unit_ptr(u, up_c), s, cur);
+#pragma unroll 1
+  while (u < nunits) {
+    const int un = u + TY;
+    if (valid && un < nunits) load_stencil<RECON>(unit_ptr(un, up_n), s, nxt);
+    if (valid) {
+      const int vr = (K == 0) ? u : (u >> 1);
+      double l, h;
+      recon_cell<RECON>(eps_w, cur[0], cur[1], cur[2], cur[3], cur[4], l, h);
+      if (vr < 2) {
+        if (!(l > 0.0)) l = cur[2];
+        if (!(h > 0.0)) h = cur[2];
+      }
+      if (up_c) S.exlo[vr][r] = l;
+      else S.ex[vr][(K == 0) ? r * EXW : r] = h;
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) cur[q] = nxt[q];
+    up_c = up_n;
+    u = un;
   }
 }
 
@@ -180,9 +236,9 @@ __device__ __forceinline__ void riemann(const GridView& G, const PencilTabs& T, 
   FaceMet m;
   load_face_met(T, K, cl, cr, m);
   // HLLE weights (Eq. 30; reading R6)
-  const double c = m.alpha * sqrt(m.gi0[0]);
+  const double c = m.alpha * sqrt_fast(m.gi0[0]);
   const double lp = fmax(0.0, c - m.b0), lm = fmin(0.0, -c - m.b0);
-  const double inv = 1.0 / (lp - lm);
+  const double inv = rcp_fast(lp - lm);
   const double wL = lp * inv, wR = -lm * inv, sd = lp * lm * inv;
   double sigL = 0.0, sigR = 0.0;
   if (CHARGE == CHARGE_FACE_OHM) { sigL = sigma_cell(G, cl); sigR = sigma_cell(G, cr); }
@@ -219,44 +275,19 @@ k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilT
       const int up = (K == 0) ? 1 : (K == 1) ? EXW : 0;                // own upper-face slot relative to base
       const long long cm = (K == 2) ? c + sz : c;                      // the cell this thread reconstructs
       double lo[NVR];
-      // ---- a2: reconstruction passes (p = 0: halo cells of the tile, designated lanes; p = 1: own cell)
-      {
-        bool ex_valid = false, ex_upper = false;
-        int ex_r = 0;
-        long long ex_cell = 0;
-        if (K == 0 && ty == TY - 1 && tx < 2 * TY) {                   // x: rows r, lower (-1, r) / upper (txn, r)
-          ex_r = tx & (TY - 1); ex_upper = tx >= TY; ex_valid = ex_r < tyn;
-          ex_cell = c + (long long)((ex_upper ? txn : -1) - tx) + sy * (long long)(ex_r - ty);
-        } else if (K == 1 && ty < 2) {                                 // y: columns tx, lower (tx, -1) / upper (tx, tyn)
-          ex_r = tx; ex_upper = ty == 1; ex_valid = tx < txn;
-          ex_cell = c + sy * (long long)((ex_upper ? tyn : -1) - ty);
-        }
-#pragma unroll 1
-        for (int p = ex_valid ? 0 : 1; p < 2; ++p) {
-          long long ct;
-          double *hd, *h2, *ld;
-          bool sth, sth2, stl, valid;
-          if (p == 0) {
-            ct = ex_cell; valid = true;
-            hd = (K == 0) ? &S.ex[0][ex_r * EXW] : &S.ex[0][ex_r]; sth = !ex_upper;
-            h2 = hd; sth2 = false;
-            ld = &S.exlo[0][ex_r]; stl = ex_upper;
-          } else {
-            ct = cm; valid = in;
-            hd = &S.ex[0][base + up]; sth = true;
-            h2 = &S.exhi[0][(K == 0) ? ty : tx]; sth2 = (K == 0) ? (tx == txn - 1) : (K == 1) ? (ty == tyn - 1) : false;
-            ld = hd; stl = false;
-          }
-          if (valid) recon_all<RECON, NV>(T, K, ct, s, G.weno_eps, lo, hd, EXP, sth, h2, sth2, ld, stl);
-        }
+      // ---- a2: reconstruction (halo cells of the tile: all warps share them; then the own cell)
+      if (K < 2) recon_halo<RECON, NV>(T, K, S, c, s, sy, G.weno_eps, tx, ty, txn, tyn);
+      if (in) {
+        const bool edge = (K == 0) ? (tx == txn - 1) : (K == 1) ? (ty == tyn - 1) : false;
+        recon_own<RECON, NV>(T, K, cm, s, G.weno_eps, lo, &S.ex[0][base + up], EXP, &S.exhi[0][(K == 0) ? ty : tx], edge);
       }
       if (K < 2) __syncthreads();                                      // A: upper-face states visible
       // ---- a3: Riemann passes (p = 0: own lower face (x, y) / upper face (z); p = 1: faces on the tile's upper edge)
       {
         bool e_valid = false;
         int e_r = 0;
-        if (K == 0 && ty == 2 && tx < tyn) { e_valid = true; e_r = tx; }
-        if (K == 1 && ty == 3 && tx < txn) { e_valid = true; e_r = tx; }
+        if (K == 0 && ty == TY - 1 && tx < tyn) { e_valid = true; e_r = tx; }
+        if (K == 1 && ty == TY - 1 && tx < txn) { e_valid = true; e_r = tx; }
 #pragma unroll 1
         for (int p = 0; p < 2; ++p) {
           bool valid;
