@@ -117,8 +117,9 @@ int rgrmhd_set_sigma(rgrmhd_t h, const double* sigma);
  * the conserved state (Eq. 22-24, 28).  Requires set_metric first. */
 int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]);
 
-/* One IMEX-SSP2(2,2,2) step of size dt (Eq. 35-37): implicit-E + recovery, ghost fill,
- * reconstruction + HLLE + divergence + sources, stage combine; twice; final recovery. */
+/* One IMEX-SSP2(2,2,2) step of size dt (Eq. 35-37): implicit-E + recovery (+ the point-wise
+ * explicit sources and stage-combine terms of that stage), ghost fill, reconstruction + HLLE +
+ * flux divergence into the stage target; twice; final recovery. */
 int rgrmhd_step(rgrmhd_t h, double dt, int scheme);
 
 /* max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k
@@ -133,12 +134,11 @@ int rgrmhd_get_cons(rgrmhd_t h, double* const cons[14]);
 int rgrmhd_get_stats(rgrmhd_t h, rgrmhd_stats* host_out);   /* synchronises */
 int rgrmhd_reset_stats(rgrmhd_t h);
 
-/* Which RHS kernel rgrmhd_step uses: 0 (default) = the pencil-tiled kernel (each cell reconstructed
- * once per direction, every face solved once, face states and fluxes exchanged on chip); 1 = the
- * simple one-thread-per-cell kernel that recomputes its six faces from global memory (kept as the
- * in-library cross-check; also used for block shapes with an inactive direction); 2 = the
- * first-generation tiled kernel (per-face reconstruction).  All three implement the same arithmetic
- * and agree to rounding. */
+/* Which flux-divergence kernel rgrmhd_step uses: 0 (default) = the pencil-tiled kernel (each cell
+ * reconstructed once per direction, every face solved once, face states and fluxes exchanged on chip);
+ * 1 = the simple one-thread-per-cell kernel that recomputes its six faces from global memory (kept as
+ * the in-library cross-check; also used for block shapes with an inactive direction).  Both implement
+ * the same arithmetic and agree to rounding. */
 int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant);
 
 /* Kernel launches enqueued by this handle since create (bench.py's "gpu_launches"). */

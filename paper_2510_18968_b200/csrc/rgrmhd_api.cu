@@ -12,12 +12,9 @@
 #include "rgrmhd_common.cuh"
 
 namespace rg {
-cudaError_t launch_c2p(const GridView& G, double* const Ust[NCONS], double* const Xout[3], double adt,
-                       bool write_back_floor, StatsDev* stats, cudaStream_t st);
+cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats, cudaStream_t st);
 cudaError_t launch_prim2cons(const GridView& G, cudaStream_t st);
 cudaError_t launch_rhs_simple(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
-cudaError_t launch_rhs_tiled(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
-bool rhs_tiled_supported(const GridView& G);
 cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 bool rhs_pencil_supported(const GridView& G);
 cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, cudaStream_t st);
@@ -36,7 +33,7 @@ struct rgrmhd_s {
   long long solves = 0;              // host-side count of cell solves enqueued
   long long launches = 0;
   bool have_metric = false, have_prims = false, have_sigma = false;
-  int rhs_variant = 0;               // 0 = pencil (default), 1 = simple, 2 = tiled (first generation)
+  int rhs_variant = 0;               // 0 = pencil (default), 1 = simple
   bool timing = false;
   struct Timed { int cls; cudaEvent_t a, b; };
   std::vector<Timed> timed;
@@ -188,7 +185,7 @@ int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream) {
 }
 
 int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant) {
-  if (!h || variant < 0 || variant > 2) return RGRMHD_E_INVALID;
+  if (!h || variant < 0 || variant > 1) return RGRMHD_E_INVALID;
   h->rhs_variant = variant;
   return RGRMHD_OK;
 }
@@ -253,7 +250,6 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   DeviceGuard guard(h->device);
   const rg::GridView& G = h->G;
   cudaStream_t st = h->stream;
-  const double gam = 1.0 - 1.0 / std::sqrt(2.0);
   const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
   double* ghost_fields[rg::NPRIM + 3];
   for (int v = 0; v < rg::NPRIM; ++v) ghost_fields[v] = G.P[v];
@@ -261,11 +257,8 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   const int nghost_fields = rg::NPRIM + (G.charge_mode == rg::CHARGE_CELL_CURRENT ? 3 : 0);
   const bool any_active = G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1;
   const bool pencil = h->rhs_variant == 0 && rg::rhs_pencil_supported(G);
-  const bool tiled = h->rhs_variant == 2 && rg::rhs_tiled_supported(G);
   auto rhs = [&](int stage) {
-    return pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, st)
-         : tiled  ? rg::launch_rhs_tiled(G, dt, stage, recon, st)
-                  : rg::launch_rhs_simple(G, dt, stage, recon, st);
+    return pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, st) : rg::launch_rhs_simple(G, dt, stage, recon, st);
   };
   // optional per-kernel event bracket (rgrmhd_set_timing)
   auto timed = [&](int cls, auto&& launch) -> cudaError_t {
@@ -281,16 +274,17 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
     h->timed.push_back(t);
     return e;
   };
-  // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n
-  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, G.Un, G.X1, gam * dt, false, h->stats_dev, st); }));
+  // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n.  The recovery kernel also applies the point-wise half of the
+  // right-hand side (sources, implicit terms) to the stage target; the flux kernel adds -w dt div F.
+  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 1, dt, h->stats_dev, st); }));
   if (any_active) RG_CUDA(h, timed(RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
   RG_CUDA(h, timed(RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
   // stage 2 (Eq. 36)
-  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, G.Us, nullptr, gam * dt, false, h->stats_dev, st); }));
+  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
   if (any_active) RG_CUDA(h, timed(RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
   RG_CUDA(h, timed(RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
   // recovery of the new state at fixed calE (reading R12)
-  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, G.Un, nullptr, 0.0, true, h->stats_dev, st); }));
+  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 3, dt, h->stats_dev, st); }));
   h->solves += 3 * nint;
   h->launches += 5 + (any_active ? 2 : 0);
   return RGRMHD_OK;

@@ -1,6 +1,8 @@
 // rgrmhd_c2p.cu -- a6: implicit Ohm's-law update of the electric field fused with the 1D
 // conservative-to-primitive recovery (Eq. 42-50), one thread per cell, all
-// iterations in registers; plus a0 (prim -> cons at set_prims).
+// iterations in registers; followed, in the same thread, by the point-wise half of the right-hand side
+// of that stage: explicit sources (a4) and the point-wise part of the stage combine (a5), which need
+// nothing but the primitives just recovered.  Also here: a0 (prim -> cons at set_prims).
 //
 // The result is DEFINED (reading R8) as the root (E, v, p) of
 //   (1+s) E - s (v.E) v + s v x B = Estar^,  s = a_ii dt alpha sigma W            [Eq. 42, R7]
@@ -8,10 +10,12 @@
 //   rho = D^/W,  p = (Gamma-1)/Gamma (Z/W^2 - rho)                                [Eq. 45-49]
 // found by eliminating E from the momentum relation for frozen scalars (s, kE = v.E) and driving the
 // scalar residual g(Z) to zero with a bracketed secant; an outer Anderson(1) fixed point updates
-// (W, kE).  The solver is written as ONE loop whose body holds exactly one residual evaluation, so
-// lanes that are in different inner/outer phases still execute the expensive part convergently;
-// the loop ends for a warp when every lane is done (warp vote).
-#include "rgrmhd_common.cuh"
+// (W, kE).  The system is tensorial, so it is solved in an orthonormal triad of the cell's gamma_ij
+// (Cholesky factor, gamma = L L^T): every dot and cross product in the loop is Euclidean and the
+// metric is touched only before and after.  The solver is ONE loop whose body holds exactly one
+// residual evaluation, so lanes in different inner/outer phases still execute the expensive part
+// convergently; the loop ends for a warp when every lane is done (warp vote).
+#include "rgrmhd_sources.cuh"
 
 namespace rg {
 
@@ -20,99 +24,94 @@ struct C2POut {
   int failed;
 };
 
-// Work in the cell's coordinate basis with explicit index placement.
-struct C2PState {
-  // constants of the cell
-  double Dh, tauh, B2, s0, gm1og;
-  double EstarU[3], BU[3], BD[3];
-  // frozen per outer pass
-  double s, kE, r;
-  double NparU[3], NperpU[3], BxNperpU[3];
-  // last evaluation
-  double vU[3], EU[3], W, rho, p;
+// Orthonormal triad of gamma_ij: lower Cholesky factor L (gamma = L L^T) and the reciprocals of its
+// diagonal.  a^ = L^T a for contravariant, a^ = L^-1 a for covariant components; a.b and a x b are then
+// Euclidean (det L > 0: the triad is right handed, so [ijk]/sqrt(gamma) -> [abc]).
+struct Triad {
+  double l11, l21, l31, l22, l32, l33, i11, i22, i33;
 };
+__device__ __forceinline__ void triad_make(const double g[6], Triad& t) {
+  sqrt_rsqrt_fast(g[0], t.l11, t.i11);
+  t.l21 = g[1] * t.i11; t.l31 = g[2] * t.i11;
+  sqrt_rsqrt_fast(g[3] - t.l21 * t.l21, t.l22, t.i22);
+  t.l32 = (g[4] - t.l31 * t.l21) * t.i22;
+  sqrt_rsqrt_fast(g[5] - t.l31 * t.l31 - t.l32 * t.l32, t.l33, t.i33);
+}
+__device__ __forceinline__ void triad_from_contra(const Triad& t, double a0, double a1, double a2, double h[3]) {
+  h[0] = t.l11 * a0 + t.l21 * a1 + t.l31 * a2;
+  h[1] = t.l22 * a1 + t.l32 * a2;
+  h[2] = t.l33 * a2;
+}
+__device__ __forceinline__ void triad_from_cov(const Triad& t, double a0, double a1, double a2, double h[3]) {
+  h[0] = a0 * t.i11;
+  h[1] = (a1 - t.l21 * h[0]) * t.i22;
+  h[2] = (a2 - t.l31 * h[0] - t.l32 * h[1]) * t.i33;
+}
+__device__ __forceinline__ void triad_to_contra(const Triad& t, const double h[3], double a[3]) {
+  a[2] = h[2] * t.i33;
+  a[1] = (h[1] - t.l32 * a[2]) * t.i22;
+  a[0] = (h[0] - t.l21 * a[1] - t.l31 * a[2]) * t.i11;
+}
+__device__ __forceinline__ void cross3(const double a[3], const double b[3], double c[3]) {
+  c[0] = a[1] * b[2] - a[2] * b[1];
+  c[1] = a[2] * b[0] - a[0] * b[2];
+  c[2] = a[0] * b[1] - a[1] * b[0];
+}
 
-// residual g(Z) for frozen (s, kE); false when v^2 >= 1 (treated as g = -infinity)
-__device__ __forceinline__ bool c2p_residual(const Met& m, C2PState& w, double Z, double& g) {
-  const double A = Z + w.r * w.B2, c = w.r * w.kE;
-  const double iden = 1.0 / (A * A + c * c * w.B2), iZ = 1.0 / Z;
-#pragma unroll
-  for (int i = 0; i < 3; ++i) w.vU[i] = w.NparU[i] * iZ + (A * w.NperpU[i] + c * w.BxNperpU[i]) * iden;
-  double vD[3];
-  lower(m, w.vU, vD);
-  const double v2 = dot3(w.vU, vD);
-  if (!(v2 < 1.0)) return false;
-  const double W2 = 1.0 / (1.0 - v2);
-  w.W = sqrt(W2);
+// closed form of Eq. 42 at fixed v (reading R7), triad components
+__device__ __forceinline__ void implicit_E_closed(const double v[3], double W, double s, const double Es[3],
+                                                  const double B[3], double E[3]) {
   double vxB[3];
-  cross_raw(vD, w.BD, vxB);                               // (v x B)^i = [ijk] v_j B_k / sg
-  const double isg = 1.0 / m.sg, i1s = 1.0 / (1.0 + w.s), skE = w.s * w.kE;
+  cross3(v, B, vxB);
+  const double kE = dot3(v, Es) / (1.0 + s / (W * W)), i1s = 1.0 / (1.0 + s);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) w.EU[i] = (w.EstarU[i] - w.s * (vxB[i] * isg) + skE * w.vU[i]) * i1s;
-  double ED[3];
-  lower(m, w.EU, ED);
-  const double E2 = dot3(w.EU, ED);
-  w.rho = w.Dh / w.W;
-  w.p = w.gm1og * (Z * (1.0 - v2) - w.rho);
-  g = Z - (w.tauh + w.Dh + w.p - 0.5 * (E2 + w.B2));
-  return true;
+  for (int i = 0; i < 3; ++i) E[i] = (Es[i] - s * vxB[i] + s * kE * v[i]) * i1s;
 }
 
-// closed form of Eq. 42 at fixed v (reading R7)
-__device__ __forceinline__ void implicit_E_closed(const Met& m, const double vU[3], double W, double s,
-                                                  const double EstarU[3], const double BD[3], double EU[3]) {
-  double vD[3], EstarD[3], vxB[3];
-  lower(m, vU, vD); lower(m, EstarU, EstarD);
-  cross_raw(vD, BD, vxB);
-  const double kE = dot3(vU, EstarD) / (1.0 + s / (W * W));
-#pragma unroll
-  for (int i = 0; i < 3; ++i) EU[i] = (EstarU[i] - s * (vxB[i] / m.sg) + s * kE * vU[i]) / (1.0 + s);
-}
-
-// P holds the guess (rho, p, v) on entry and all 14 primitives on return.
-__device__ C2POut c2p_solve(const Met& m, double Gamma, const double U[NCONS], double adt, double sigma,
-                            double tol, int maxit, double P[NPRIM]) {
-  C2PState w;
-  const double isg = 1.0 / m.sg;
-  w.gm1og = (Gamma - 1.0) / Gamma;
-  w.Dh = U[CD] * isg; w.tauh = U[CTAU] * isg;
-  const double ShD[3] = {U[CSX] * isg, U[CSY] * isg, U[CSZ] * isg};
-  double ShU[3], EstarD[3], EsxB[3];
-  raise(m, ShD, ShU);
-#pragma unroll
-  for (int i = 0; i < 3; ++i) { w.EstarU[i] = U[CEX + i] * isg; w.BU[i] = U[CBX + i] * isg; }
-  lower(m, w.BU, w.BD); lower(m, w.EstarU, EstarD);
-  w.B2 = dot3(w.BU, w.BD);
-  cross_raw(EstarD, w.BD, EsxB);
-#pragma unroll
-  for (int i = 0; i < 3; ++i) EsxB[i] *= isg;              // (E* x B)^i
-  w.s0 = adt * m.alpha * sigma;
-  const double s0 = w.s0;
-  const double escale = sqrt(dot3(w.EstarU, EstarD) + w.B2);
-  C2POut res = {0, 1};
+// P holds the guess (rho, p, v^i) on entry and all 14 primitives on return.  sg = sqrt(gamma).
+__device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double alpha, double Gamma,
+                                            const double U[NCONS], double adt, double sigma, double tol, int maxit,
+                                            double P[NPRIM]) {
+  const double isg = rcp_fast(sg);
+  const double gm1og = (Gamma - 1.0) / Gamma;
+  const double Dh = U[CD] * isg, tauh = U[CTAU] * isg;
+  double Sh[3], Es[3], B[3], EsxB[3];
+  triad_from_cov(t, U[CSX] * isg, U[CSY] * isg, U[CSZ] * isg, Sh);
   // EM fields that do not depend on the solve
 #pragma unroll
-  for (int i = 0; i < 3; ++i) P[BX + i] = w.BU[i];
+  for (int i = 0; i < 3; ++i) P[BX + i] = U[CBX + i] * isg;
   P[PSI] = U[CPSI] * isg; P[PHI] = U[CPHI] * isg; P[QCH] = U[CQ] * isg;
-  const double Zlo = w.Dh, Zhi = Gamma * (w.tauh + w.Dh - 0.5 * w.B2);
+  triad_from_contra(t, U[CEX] * isg, U[CEY] * isg, U[CEZ] * isg, Es);
+  triad_from_contra(t, P[BX], P[BY], P[BZ], B);
+  const double B2 = dot3(B, B);
+  cross3(Es, B, EsxB);
+  const double s0 = adt * alpha * sigma;
+  const double escale = sqrt(dot3(Es, Es) + B2);
+  C2POut res = {0, 1};
+  const double Zlo = Dh, Zhi = Gamma * (tauh + Dh - 0.5 * B2);
   // guess
-  double vgU[3] = {P[VX], P[VY], P[VZ]}, vgD[3];
-  lower(m, vgU, vgD);
-  double v2g = dot3(vgU, vgD);
-  if (!(v2g < 1.0)) { vgU[0] = vgU[1] = vgU[2] = 0.0; v2g = 0.0; }
-  const double Wg = 1.0 / sqrt(1.0 - v2g);
+  double vg[3];
+  triad_from_contra(t, P[VX], P[VY], P[VZ], vg);
+  double v2g = dot3(vg, vg);
+  if (!(v2g < 1.0)) { vg[0] = vg[1] = vg[2] = 0.0; v2g = 0.0; }
+  const double Wg = rsqrt_fast(1.0 - v2g);
   double W = Wg;
-  double kE = dot3(vgU, EstarD) / (1.0 + s0 / W);
-  if (!(w.Dh > 0.0) || !(Zhi > Zlo)) {   // no physical bracket: keep the guess, E from the guess v
-    double EU[3];
-    implicit_E_closed(m, vgU, W, s0 * W, w.EstarU, w.BD, EU);
+  double kE = dot3(vg, Es) * W * rcp_fast(W + s0);          // (v.E*)/(1 + s/W^2), s = s0 W
+  if (!(Dh > 0.0) || !(Zhi > Zlo)) {   // no physical bracket: keep the guess, E from the guess v
+    double Eh[3], EU[3];
+    implicit_E_closed(vg, W, s0 * W, Es, B, Eh);
+    triad_to_contra(t, Eh, EU);
     P[EX] = EU[0]; P[EY] = EU[1]; P[EZ] = EU[2];
     return res;
   }
   double Z = (P[RHO] + Gamma / (Gamma - 1.0) * P[PRS]) * W * W;
   bool converged = false, state_ok = false;
   const int max_outer = 50;
-  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, slope = 1.0;
+  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, islope = 1.0;
+  // frozen per outer pass
+  double s = 0, r = 0, i1s = 1, Npar[3] = {0, 0, 0}, Nperp[3] = {0, 0, 0}, BxN[3] = {0, 0, 0};
+  // last evaluation
+  double v[3] = {0, 0, 0}, E[3] = {0, 0, 0}, Wv = 1, rho = 0, p = 0;
   // inner-loop state
   double a = Zlo, b = Zhi, x = Z, f = 0, xp = 0, fp = 0;
   bool ok = false, okp = false;
@@ -123,26 +122,39 @@ __device__ C2POut c2p_solve(const Met& m, double Gamma, const double U[NCONS], d
     if (!done) {
       if (need_setup) {
         // ---- outer pass set-up: freeze (s, kE), decompose N along/across B ---------------------
-        w.s = s0 * W; w.r = w.s / (1.0 + w.s); w.kE = kE;
-        double NU[3], ND[3], NperpD[3];
-        const double i1s = 1.0 / (1.0 + w.s);
+        s = s0 * W; i1s = rcp_fast(1.0 + s); r = s * i1s;
+        double N[3];
 #pragma unroll
-        for (int i = 0; i < 3; ++i) NU[i] = ShU[i] - EsxB[i] * i1s;
-        lower(m, NU, ND);
-        const double NdotB = dot3(NU, w.BD);
-        const double fpar = (w.B2 > 0.0) ? NdotB / w.B2 : 0.0;
+        for (int i = 0; i < 3; ++i) N[i] = Sh[i] - EsxB[i] * i1s;
+        const double fpar = (B2 > 0.0) ? dot3(N, B) / B2 : 0.0;
 #pragma unroll
-        for (int i = 0; i < 3; ++i) { w.NparU[i] = fpar * w.BU[i]; w.NperpU[i] = NU[i] - w.NparU[i]; }
-        lower(m, w.NperpU, NperpD);
-        cross_raw(w.BD, NperpD, w.BxNperpU);
-#pragma unroll
-        for (int i = 0; i < 3; ++i) w.BxNperpU[i] *= isg;
+        for (int i = 0; i < 3; ++i) { Npar[i] = fpar * B[i]; Nperp[i] = N[i] - Npar[i]; }
+        cross3(B, Nperp, BxN);
         a = Zlo; b = Zhi;
         x = fmin(fmax(Z, a), b);
         okp = false;
         need_setup = false;
       }
-      ok = c2p_residual(m, w, x, f);
+      // ---- residual g(x) for frozen (s, kE); v^2 >= 1 counts as g = -infinity ------------------
+      {
+        const double A = x + r * B2, c = r * kE;
+        const double iden = rcp_fast(A * A + c * c * B2), iZ = rcp_fast(x);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) v[i] = Npar[i] * iZ + (A * Nperp[i] + c * BxN[i]) * iden;
+        const double v2 = dot3(v, v);
+        ok = v2 < 1.0;
+        const double omv2 = ok ? 1.0 - v2 : 1.0;
+        double iW;
+        sqrt_rsqrt_fast(omv2, iW, Wv);                                   // 1/W, W
+        double vxB[3];
+        cross3(v, B, vxB);
+        const double skE = s * kE;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) E[i] = (Es[i] - s * vxB[i] + skE * v[i]) * i1s;
+        rho = Dh * iW;                                                   // Eq. 45
+        p = gm1og * (x * omv2 - rho);                                    // Eq. 47-49
+        f = x - (tauh + Dh + p - 0.5 * (dot3(E, E) + B2));
+      }
       ++res.evals;
       // ---- inner: bracketed secant / bisection on Z; invariant g(a) < 0 < g(b) -----------------
       bool inner_conv = false, inner_stop = false;
@@ -150,8 +162,10 @@ __device__ C2POut c2p_solve(const Met& m, double Gamma, const double U[NCONS], d
         inner_conv = true;
       } else {
         if (!ok || f < 0.0) a = x; else b = x;
-        if (ok && okp && f != fp && x != xp) slope = (f - fp) / (x - xp);
-        const double delta = ok ? f / slope : 0.0;          // predicted distance to the root
+        const bool sec = ok && okp && f != fp && x != xp;
+        const double isl = (x - xp) * rcp_fast(sec ? f - fp : 1.0);
+        if (sec) islope = isl;
+        const double delta = ok ? f * islope : 0.0;          // predicted distance to the root
         if (ok && fabs(delta) <= tol * fabs(x)) inner_conv = true;
         else if (ok && (b - a) <= tol * fabs(x)) inner_conv = true;
         else if (res.evals >= maxit) inner_stop = true;
@@ -168,8 +182,8 @@ __device__ C2POut c2p_solve(const Met& m, double Gamma, const double U[NCONS], d
           done = true;
         } else {
           // ---- outer: update (s, kE) from the new v ------------------------------------------------
-          const double Wnew = w.W;
-          const double kEnew = dot3(w.vU, EstarD) / (1.0 + s0 / Wnew);
+          const double Wnew = Wv;
+          const double kEnew = dot3(v, Es) * Wnew * rcp_fast(Wnew + s0);
           const bool same = fabs(Wnew - W) <= tol * Wnew && fabs(kEnew - kE) <= tol * escale;
           if (s0 == 0.0 || same) {
             converged = true; done = true;
@@ -198,73 +212,91 @@ __device__ C2POut c2p_solve(const Met& m, double Gamma, const double U[NCONS], d
     if (__all_sync(__activemask(), done)) break;            // warp-vote exit
   }
   res.failed = converged ? 0 : 1;
+  double EU[3];
   if (state_ok) {
-    P[RHO] = w.rho; P[PRS] = w.p;
+    double vU[3];
+    triad_to_contra(t, v, vU);
+    triad_to_contra(t, E, EU);
+    P[RHO] = rho; P[PRS] = p;
 #pragma unroll
-    for (int i = 0; i < 3; ++i) { P[VX + i] = w.vU[i]; P[EX + i] = w.EU[i]; }
+    for (int i = 0; i < 3; ++i) P[VX + i] = vU[i];
   } else {
-    double EU[3];
-    implicit_E_closed(m, vgU, Wg, s0 * Wg, w.EstarU, w.BD, EU);
-    P[EX] = EU[0]; P[EY] = EU[1]; P[EZ] = EU[2];
+    double Eh[3];
+    implicit_E_closed(vg, Wg, s0 * Wg, Es, B, Eh);
+    triad_to_contra(t, Eh, EU);
   }
+  P[EX] = EU[0]; P[EY] = EU[1]; P[EZ] = EU[2];
   return res;
 }
 
-// a6 over the grid.  Ust = stage vector (its calE entries are X*), guess = current G.P.  Writes G.P,
-// the conduction current G.jc (reading R3) and, if Xout != null, the stage calE = sqrt(gamma) E.
-// Floor rule: reading R9; write_back_floor only in the final recovery of a step.
-struct C2PArgs {
-  double* Ust[NCONS];
-  double* Xout[3];
-  double adt;
-  int write_back_floor;
-  int has_xout;
-};
+// a6 (+ a4, a5 point-wise) over the grid.
+//   STAGE 1: stage vector U^n (X*1 = X^n),  a = gamma dt; writes P, jc, X1 and the bracket of U*2 into G.Us
+//   STAGE 2: stage vector U*2 (G.Us),       a = gamma dt; writes P, jc and the bracket of U^{n+1} into G.Un
+//   STAGE 3: recovery of U^{n+1} (G.Un) at fixed calE (a = 0, reading R12); writes P; floor write-back (R9)
+// The guess is the current G.P.  jc = undensitised conduction current of the stage (reading R3).
+constexpr int C2P_TX = 32, C2P_TY = 4;
 
-__global__ void __launch_bounds__(128)
-k_c2p(const __grid_constant__ GridView G, const __grid_constant__ C2PArgs A, StatsDev* __restrict__ stats) {
-  const int nx = G.n[0], ny = G.n[1];
-  const long long nint = (long long)nx * ny * G.n[2];
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+template <int STAGE>
+__global__ void __launch_bounds__(C2P_TX * C2P_TY, 3)
+k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stats) {
+  const int i = blockIdx.x * C2P_TX + (threadIdx.x & (C2P_TX - 1));
+  const int j = blockIdx.y * C2P_TY + (threadIdx.x / C2P_TX);
+  const int k = blockIdx.z;
+  const double gam = 1.0 - 0.70710678118654752440;   // 1 - 1/sqrt(2) (Eq. 35-37)
+  const double adt = (STAGE == 3) ? 0.0 : gam * dt;
+  double* const* Ust = (STAGE == 2) ? G.Us : G.Un;
   int evals = 0, failed = 0, floored = 0;
-  if (t < nint) {
-    const int i = (int)(t % nx);
-    const long long r = t / nx;
-    const int j = (int)(r % ny), k = (int)(r / ny);
+  if (i < G.n[0] && j < G.n[1]) {
     const long long c = cell_index(G, i, j, k);
-    Met m;
-    load_met_cell(G, c, m);
+    double g6[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) g6[q] = __ldg(G.met[MGXX + q] + c);
+    const double alpha = __ldg(G.met[MALP] + c);
+    Triad t;
+    triad_make(g6, t);
+    const double sg = t.l11 * t.l22 * t.l33;
     double U[NCONS], P[NPRIM];
 #pragma unroll
-    for (int v = 0; v < NCONS; ++v) U[v] = A.Ust[v][c];
+    for (int v = 0; v < NCONS; ++v) U[v] = Ust[v][c];
 #pragma unroll
     for (int v = 0; v < 5; ++v) P[v] = G.P[v][c];
-    const double Dh = U[CD] / m.sg;
-    const double sigma = (A.adt > 0.0) ? sigma_of(G, Dh, c) : 0.0;
-    C2POut r2 = c2p_solve(m, G.Gamma, U, A.adt, sigma, G.tol, G.maxit, P);
+    const double sigma = (STAGE == 3) ? 0.0 : sigma_of(G, U[CD] / sg, c);
+    C2POut r2 = c2p_solve(t, sg, alpha, G.Gamma, U, adt, sigma, G.tol, G.maxit, P);
     evals = r2.evals; failed = r2.failed;
     if (G.rho_floor > 0.0 && (r2.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
       // reading R9: atmosphere reset
       floored = 1;
       P[RHO] = G.rho_floor; P[VX] = P[VY] = P[VZ] = 0.0;
       P[PRS] = G.p_atmo;
-      const double s = A.adt * m.alpha * sigma;
+      const double s = adt * alpha * sigma;
 #pragma unroll
-      for (int q = 0; q < 3; ++q) P[EX + q] = (U[CEX + q] / m.sg) / (1.0 + s);
-      if (A.write_back_floor) {
+      for (int q = 0; q < 3; ++q) P[EX + q] = (U[CEX + q] / sg) / (1.0 + s);
+      if (STAGE == 3) {
+        Met m;
+        load_met_cell(G, c, m);
         double Unew[NCONS];
         prim2cons(m, G.Gamma, P, Unew);
-        A.Ust[CD][c] = Unew[CD]; A.Ust[CTAU][c] = Unew[CTAU];
+        Ust[CD][c] = Unew[CD]; Ust[CTAU][c] = Unew[CTAU];
 #pragma unroll
-        for (int q = 0; q < 3; ++q) A.Ust[CSX + q][c] = Unew[CSX + q];
+        for (int q = 0; q < 3; ++q) Ust[CSX + q][c] = Unew[CSX + q];
       }
     }
 #pragma unroll
     for (int v = 0; v < NPRIM; ++v) G.P[v][c] = P[v];
+    double sgE[3];
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
-      if (A.has_xout) A.Xout[q][c] = m.sg * P[EX + q];
-      G.jc[q][c] = (A.adt > 0.0) ? (U[CEX + q] / m.sg - P[EX + q]) / (A.adt * m.alpha) : 0.0;
+      sgE[q] = sg * P[EX + q];
+      if (STAGE == 1) G.X1[q][c] = sgE[q];
+      G.jc[q][c] = (STAGE == 3) ? 0.0 : (U[CEX + q] / sg - P[EX + q]) / (adt * alpha);
+    }
+    if (STAGE != 3) {
+      // ---- a4 + a5 (point-wise part)
+      double S[NCONS];
+#pragma unroll
+      for (int v = 0; v < NCONS; ++v) S[v] = 0.0;
+      add_sources(G, c, P, S);
+      stage_precombine<STAGE>(G, c, dt, S, sgE);
     }
   }
   // stats: warp reduce, one atomic per warp
@@ -301,16 +333,13 @@ k_prim2cons(const __grid_constant__ GridView G) {
 }
 
 // ---- launchers -----------------------------------------------------------------------------------
-cudaError_t launch_c2p(const GridView& G, double* const Ust[NCONS], double* const Xout[3], double adt,
-                       bool write_back_floor, StatsDev* stats, cudaStream_t st) {
-  C2PArgs A;
-  for (int v = 0; v < NCONS; ++v) A.Ust[v] = Ust[v];
-  for (int q = 0; q < 3; ++q) A.Xout[q] = Xout ? Xout[q] : nullptr;
-  A.adt = adt; A.write_back_floor = write_back_floor ? 1 : 0; A.has_xout = Xout ? 1 : 0;
-  const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
-  const int threads = 128;
-  const unsigned blocks = (unsigned)((nint + threads - 1) / threads);
-  k_c2p<<<blocks, threads, 0, st>>>(G, A, stats);
+cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats, cudaStream_t st) {
+  const dim3 block(C2P_TX * C2P_TY, 1, 1);
+  const dim3 grid((G.n[0] + C2P_TX - 1) / C2P_TX, (G.n[1] + C2P_TY - 1) / C2P_TY, G.n[2]);
+  if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
+  if (stage == 1) k_c2p<1><<<grid, block, 0, st>>>(G, dt, stats);
+  else if (stage == 2) k_c2p<2><<<grid, block, 0, st>>>(G, dt, stats);
+  else k_c2p<3><<<grid, block, 0, st>>>(G, dt, stats);
   return cudaGetLastError();
 }
 

@@ -1,5 +1,6 @@
-// rgrmhd_rhs_pencil.cu -- the production RHS kernel (a2-a5): reconstruct + HLLE + flux divergence +
-// explicit sources + IMEX stage combine in ONE launch.  Face states and fluxes never leave the SM.
+// rgrmhd_rhs_pencil.cu -- flux-divergence kernel (a2, a3, divergence of a4, divergence part of a5):
+// reconstruct + HLLE + flux divergence + update of the stage target in ONE launch.  Face states and fluxes
+// never leave the SM.  (The point-wise sources and the rest of the stage combine run in the recovery kernel.)
 //
 // Decomposition ("pencil-tiled"): a CTA owns a TX x TY (x, y) tile of z-pencils and marches CZ planes
 // along z; one thread = one cell of the current plane.  Per plane, for each direction K (x, y, z):
@@ -13,7 +14,7 @@
 //       and its neighbour's flux.  No face is solved twice except the TX + TY faces on the tile's
 //       upper x / y edge, which one warp each handles in an extra pass (their reconstruction halo:
 //       two more partial warps).
-//   a4, a5  geometric sources, stage combine, one store of U*2 / U^{n+1}.
+//   a5  U*2 += dt dU or U^{n+1} += dt/2 dU (one read-modify-write of the stage target).
 // The three directions run through ONE copy of the reconstruction and Riemann code: direction K is a
 // run-time cyclic rotation of the vector/tensor components (cyclic permutations keep the Levi-Civita
 // sign, so Eq. 27 is form invariant), realised for free as index arithmetic on pointer tables and
@@ -339,19 +340,7 @@ k_rhs_pencil(const __grid_constant__ GridView G, const __grid_constant__ PencilT
         dU[v] = S.du[v][tid] - Fz;
         S.du[v][tid] = Fz;                                             // lower z face of the next plane
       }
-      if (k >= k0) {
-        // ---- a4 + a5
-        double P[NPRIM];
-#pragma unroll
-        for (int v = 0; v < NPRIM; ++v) P[v] = G.P[v][c];
-        add_sources(G, c, P, dU);
-        Met m;
-#pragma unroll
-        for (int q = 0; q < 6; ++q) m.g[q] = __ldg(G.met[MGXX + q] + c);
-        met_finish(m);
-        const double sgE[3] = {m.sg * P[EX], m.sg * P[EY], m.sg * P[EZ]};
-        stage_combine<STAGE>(G, c, dt, dU, sgE);
-      }
+      if (k >= k0) divergence_update<STAGE>(G, c, dt, dU);             // a5 (divergence part)
     }
     __syncthreads();                                                   // D: exchange buffer free for the next plane
   }

@@ -1,9 +1,9 @@
-// rgrmhd_rhs_simple.cu -- reference-quality RHS kernel (a2-a5): one thread per interior cell, each
-// thread evaluates the HLLE flux at all of its (up to six) faces straight from global memory.  Every
-// face is therefore computed twice; this kernel exists as the simplest correct CUDA statement of the
-// RHS (selected with RGRMHD_RHS_SIMPLE=1 or for shapes the tiled kernel does not cover) and as the
-// in-library cross-check of the tiled kernel in rgrmhd_rhs_tiled.cu.  Also here: a1 ghost fill and
-// a7 max-speed reduction.
+// rgrmhd_rhs_simple.cu -- reference-quality flux-divergence kernel (a2, a3, divergence): one thread per
+// interior cell, each thread evaluates the HLLE flux at all of its (up to six) faces straight from global
+// memory.  Every face is therefore computed twice; this kernel exists as the simplest correct CUDA
+// statement of the flux divergence (rgrmhd_set_rhs_variant(1), and block shapes with an inactive
+// direction) and as the in-library cross-check of the tiled kernels.  Also here: a1 ghost fill and a7
+// max-speed reduction.
 #include "rgrmhd_rhs.cuh"
 
 namespace rg {
@@ -41,20 +41,7 @@ k_rhs_simple(const __grid_constant__ GridView G, double dt) {
 #pragma unroll
     for (int v = 0; v < NCONS; ++v) F[v] -= (Fp[v] - Fm[v]) * G.inv_dx[2];
   }
-  double P[NPRIM];
-#pragma unroll
-  for (int v = 0; v < NPRIM; ++v) P[v] = G.P[v][c];
-  add_sources(G, c, P, F);
-  // sqrt(gamma) E of this stage (X^(stage), Eq. 35-36)
-  double g6[6];
-#pragma unroll
-  for (int q = 0; q < 6; ++q) g6[q] = __ldg(G.met[MGXX + q] + c);
-  Met m;
-#pragma unroll
-  for (int q = 0; q < 6; ++q) m.g[q] = g6[q];
-  met_finish(m);
-  const double sgE[3] = {m.sg * P[EX], m.sg * P[EY], m.sg * P[EZ]};
-  stage_combine<STAGE>(G, c, dt, F, sgE);
+  divergence_update<STAGE>(G, c, dt, F);
 }
 
 template <int RECON, int CHARGE>
