@@ -134,11 +134,13 @@ int rgrmhd_get_cons(rgrmhd_t h, double* const cons[14]);
 int rgrmhd_get_stats(rgrmhd_t h, rgrmhd_stats* host_out);   /* synchronises */
 int rgrmhd_reset_stats(rgrmhd_t h);
 
-/* Which flux-divergence kernel rgrmhd_step uses: 0 (default) = the pencil-tiled kernel (each cell
- * reconstructed once per direction, every face solved once, face states and fluxes exchanged on chip);
- * 1 = the simple one-thread-per-cell kernel that recomputes its six faces from global memory (kept as
- * the in-library cross-check; also used for block shapes with an inactive direction).  Both implement
- * the same arithmetic and agree to rounding. */
+/* Which flux-divergence kernel rgrmhd_step uses: 0 (default) = the TMA-staged tiled kernel (stencils
+ * staged in shared memory by bulk tensor copies, each cell reconstructed once per direction, every face
+ * solved once, face states and fluxes exchanged on chip; needs three active directions and an even row
+ * pitch, otherwise falls back to 2); 1 = the simple one-thread-per-cell kernel that recomputes its six
+ * faces from global memory (the in-library cross-check; also used for block shapes with an inactive
+ * direction); 2 = the pencil-tiled kernel that reads its stencils straight from global memory.  All
+ * implement the same arithmetic and agree to rounding. */
 int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant);
 
 /* Kernel launches enqueued by this handle since create (bench.py's "gpu_launches"). */

@@ -17,6 +17,9 @@ cudaError_t launch_prim2cons(const GridView& G, cudaStream_t st);
 cudaError_t launch_rhs_simple(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 bool rhs_pencil_supported(const GridView& G);
+cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int stage, int recon, cudaStream_t st);
+void* tma_create(const GridView& G);
+void tma_destroy(void* state);
 cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, cudaStream_t st);
 cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, cudaStream_t st);
 }  // namespace rg
@@ -33,7 +36,8 @@ struct rgrmhd_s {
   long long solves = 0;              // host-side count of cell solves enqueued
   long long launches = 0;
   bool have_metric = false, have_prims = false, have_sigma = false;
-  int rhs_variant = 0;               // 0 = pencil (default), 1 = simple
+  int rhs_variant = 0;               // 0 = TMA-staged (default), 1 = simple, 2 = pencil (global-memory stencils)
+  void* tma = nullptr;               // tensor maps of the TMA-staged flux kernel (null: shape not supported)
   bool timing = false;
   struct Timed { int cls; cudaEvent_t a, b; };
   std::vector<Timed> timed;
@@ -161,6 +165,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   for (int v = 0; v < 3; ++v) G.X1[v] = next();
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(h->slab); cudaFree(h->stats_dev); delete h; return RGRMHD_E_CUDA; }
+  h->tma = rg::tma_create(G);
   *out = h;
   return RGRMHD_OK;
 }
@@ -173,6 +178,7 @@ int rgrmhd_destroy(rgrmhd_t h) {
     for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(h->slab);
     cudaFree(h->stats_dev);
+    rg::tma_destroy(h->tma);
   }
   delete h;
   return RGRMHD_OK;
@@ -185,7 +191,7 @@ int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream) {
 }
 
 int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant) {
-  if (!h || variant < 0 || variant > 1) return RGRMHD_E_INVALID;
+  if (!h || variant < 0 || variant > 2) return RGRMHD_E_INVALID;
   h->rhs_variant = variant;
   return RGRMHD_OK;
 }
@@ -256,9 +262,12 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   for (int q = 0; q < 3; ++q) ghost_fields[rg::NPRIM + q] = G.jc[q];
   const int nghost_fields = rg::NPRIM + (G.charge_mode == rg::CHARGE_CELL_CURRENT ? 3 : 0);
   const bool any_active = G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1;
-  const bool pencil = h->rhs_variant == 0 && rg::rhs_pencil_supported(G);
+  const bool tma = h->rhs_variant == 0 && h->tma != nullptr;
+  const bool pencil = !tma && h->rhs_variant != 1 && rg::rhs_pencil_supported(G);
   auto rhs = [&](int stage) {
-    return pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, st) : rg::launch_rhs_simple(G, dt, stage, recon, st);
+    return tma    ? rg::launch_rhs_tma(G, h->tma, dt, stage, recon, st)
+         : pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, st)
+                  : rg::launch_rhs_simple(G, dt, stage, recon, st);
   };
   // optional per-kernel event bracket (rgrmhd_set_timing)
   auto timed = [&](int cls, auto&& launch) -> cudaError_t {

@@ -1,0 +1,409 @@
+// rgrmhd_rhs_tma.cu -- the production flux-divergence kernel (a2, a3, divergence of a4, divergence part
+// of a5) for sm_100a: reconstruct + HLLE + flux divergence + update of the stage target in ONE launch,
+// with every reconstruction stencil staged in shared memory by the TMA engine.
+//
+// Decomposition: a CTA owns a TX x TY (x, y) tile of z-pencils and marches CZ planes along z; one
+// compute thread = one cell of the current plane.  Per plane and direction K (x, y, z), for each of the
+// 15 reconstructed variables, ONE bulk tensor copy (cp.async.bulk.tensor.4d, box = the tile plus its
+// 3-cell halo along K only: (TX+6) x TY, (TX+2) x (TY+6) or (TX+2) x TY x 5 planes) lands in a ring of NS
+// shared-memory stages.  A producer warp runs the ring ahead of the compute warps (full / empty
+// mbarriers per stage), so no compute warp ever waits on a global load for a stencil:
+//   a2  every compute thread reconstructs ITS OWN CELL along K from the staged box: the smoothness
+//       indicators are computed once and give the value at the cell's lower face (registers: the right
+//       state of that face) and at its upper face (shared memory: the left state of the neighbour's
+//       face; along z it is carried to the next plane in a thread-private slot).  The 2 x 16 halo cells
+//       of the tile are reconstructed by one warp per variable (round robin), from the same box.
+//   a3  every compute thread solves the HLLE problem at its cell's lower face (x, y) / upper face (z);
+//       the TX + TY faces on the tile's upper x / y edge are solved by a helper warp, concurrently.
+//       Fluxes are exchanged through a second shared-memory buffer, so a phase needs two barriers.
+//   a5  U*2 += dt dU or U^{n+1} += dt/2 dU (one read-modify-write of the stage target, prefetched).
+// The face metric (two cells x 8 fields) is prefetched into registers before the reconstruction loop.
+// Warp roles: 8 compute warps, 1 producer warp (one lane issues the TMA copies), 1 edge-face warp.
+// The three directions run through ONE copy of the code (rgrmhd_flux_rot.cuh).
+#include <cuda.h>
+
+#include "rgrmhd_flux_rot.cuh"
+
+namespace rg {
+
+namespace {
+constexpr int TX = 16, TY = 16, NT = TX * TY;
+constexpr int NWC = NT / 32;                       // compute warps
+constexpr int NTHREADS = NT + 64;                  // + producer warp + edge-face warp
+constexpr int EXW = TX + 1, EXH = TY + 1, EXP = EXW * EXH;
+constexpr int NS = 6;                              // ring stages
+// The TMA engine needs a 16-byte aligned box origin (an even x coordinate for doubles: an odd one traps with
+// "illegal instruction"), and the ghost offset is 3: the y and z boxes therefore start one cell left of the tile
+// and are TX + 2 wide.
+constexpr int PY = TX + 2;                         // row pitch of the y and z boxes
+constexpr int BOX_X = (TX + 6) * TY, BOX_Y = PY * (TY + 6), BOX_Z = PY * TY * 5;   // doubles per box
+constexpr int STAGE_DBL = BOX_Z;
+static_assert(BOX_X <= STAGE_DBL && BOX_Y <= STAGE_DBL, "stage must hold every box");
+static_assert(TX == 16 && TY == 16, "halo / edge lane mapping assumes 16-lane rows and columns");
+
+struct Smem {
+  double ring[NS][STAGE_DBL];   // TMA destinations (128-byte aligned: STAGE_DBL * 8 is a multiple of 128)
+  double ex[NVR][EXP];          // upper-face states of the tile's cells (+ lower halo): left states of the faces
+  double fx[NCONS][EXP];        // face fluxes (slot = the cell whose lower face it is; column TX / row TY = edge)
+  double exlo[NVR][16];         // lower-face states of the upper-halo cells (right states of the edge faces)
+  double exhi[NVR][16];         // upper-face states of the last row/column (left states of the edge faces)
+  double chi[NVR][NT];          // z carry: upper-face states of the current plane
+  double du[NCONS][NT];         // flux divergence being accumulated for the current plane (thread-private)
+  unsigned long long full[NS], empty[NS];
+};
+
+struct TmaMaps {
+  CUtensorMap x, y, z;
+};
+
+// ---- mbarrier / TMA PTX ---------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+  const unsigned a = smem_u32(b);
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "W_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra D_%=;\n"
+      "bra W_%=;\n"
+      "D_%=:\n"
+      "}\n" ::"r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(const CUtensorMap* map, void* dst, unsigned long long* bar, int c0, int c1,
+                                            int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+// barrier among the compute warps and the edge-face warp (the producer warp never joins)
+__device__ __forceinline__ void bar_work() { asm volatile("bar.sync 1, %0;" ::"n"(NT + 32) : "memory"); }
+// pin a prefetched value in its register until here (keeps the consumer arithmetic below this point)
+__device__ __forceinline__ void pin(double& x) { asm volatile("" : "+d"(x)); }
+
+// rotated -> natural conserved index for K = 2 (rotated components 0,1,2 = z,x,y), known at compile time
+__host__ __device__ constexpr int nat_z(int v) {
+  return (v >= CSX && v <= CSZ) ? CSX + (v - CSX + 2) % 3
+       : (v >= CEX && v <= CEZ) ? CEX + (v - CEX + 2) % 3
+       : (v >= CBX && v <= CBZ) ? CBX + (v - CBX + 2) % 3 : v;
+}
+
+template <int RECON>
+__device__ __forceinline__ void lds_stencil(const double* __restrict__ p, int s, double u[5]) {
+  if (RECON == RECON_WENO5) { u[0] = p[-2 * s]; u[4] = p[2 * s]; } else { u[0] = 0.0; u[4] = 0.0; }
+  u[1] = p[-s]; u[2] = p[0]; u[3] = p[s];
+}
+}  // namespace
+
+template <int RECON, int CHARGE, int STAGE>
+__global__ void __launch_bounds__(NTHREADS, 1)
+k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTabs T,
+           const __grid_constant__ TmaMaps M, double dt, int CZ) {
+  constexpr int NV = (CHARGE == CHARGE_CELL_CURRENT) ? NVR : NVR - 1;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Smem& S = *reinterpret_cast<Smem*>(smem_raw);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  const int txn = min(TX, G.n[0] - i0), tyn = min(TY, G.n[1] - j0);   // valid extent of this tile
+  const int k0 = blockIdx.z * CZ, k1 = min(k0 + CZ, G.n[2]);
+  const long long sy = G.stride[1], sz = G.stride[2];
+  if (tid == 0) {
+#pragma unroll
+    for (int q = 0; q < NS; ++q) { mbar_init(&S.full[q], 1); mbar_init(&S.empty[q], NWC); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  // =================================================================================================
+  // producer warp: one lane walks the (plane, direction, variable) sequence NS boxes ahead
+  // =================================================================================================
+  if (warp == NWC) {
+    if (lane == 0) {
+      int seq = 0;
+      for (int k = k0 - 2; k < k1; ++k) {
+        for (int K = (k < k0) ? 2 : 0; K < 3; ++K) {
+          const CUtensorMap* map = (K == 0) ? &M.x : (K == 1) ? &M.y : &M.z;
+          const unsigned bytes = 8u * (unsigned)((K == 0) ? BOX_X : (K == 1) ? BOX_Y : BOX_Z);
+          // padded coordinates of the box origin (ghost offset 3): x box starts 3 cells left of the tile,
+          // y box 3 rows below, z box at plane k-1 (stencil of cell k+1: planes k-1 .. k+3); y, z boxes start
+          // one cell left of the tile (even x coordinate)
+          const int px = i0 + ((K == 0) ? 0 : 2), py = j0 + ((K == 1) ? 0 : 3), pz = k + ((K == 2) ? 2 : 3);
+          for (int vr = 0; vr < NV; ++vr, ++seq) {
+            const int st = seq % NS, it = seq / NS;
+            if (it > 0) mbar_wait(&S.empty[st], (unsigned)(it - 1) & 1u);
+            mbar_expect_tx(&S.full[st], bytes);
+            tma_load_4d(map, S.ring[st], &S.full[st], px, py, pz, T.fld[K][vr]);
+          }
+        }
+      }
+    }
+    __syncwarp();   // the idle lanes stay resident until the issuing lane is done
+    return;
+  }
+
+  // =================================================================================================
+  // edge-face warp: the TY faces on the tile's upper x edge and the TX faces on its upper y edge
+  // =================================================================================================
+  if (warp == NWC + 1) {
+    const int r = lane & 15;
+    for (int k = k0; k < k1; ++k) {
+#pragma unroll 1
+      for (int K = 0; K < 2; ++K) {
+        const bool valid = lane < 16 && r < ((K == 0) ? tyn : txn);
+        const long long cr = (K == 0) ? cell_index(G, i0 + txn, j0 + r, k) : cell_index(G, i0 + r, j0 + tyn, k);
+        const long long cl = cr - G.stride[K];
+        FaceRaw raw;
+        if (valid) load_face_raw(T, K, cl, cr, raw);
+        bar_work();                                                    // A: face states visible
+        if (valid) {
+          double PR[NVR], F[NCONS];
+#pragma unroll
+          for (int vr = 0; vr < NV; ++vr) PR[vr] = S.exlo[vr][r];
+          FaceMet m;
+          finish_face_met(raw, m);
+          riemann_m<CHARGE, NV>(G, m, cl, cr, &S.exhi[0][r], 16, PR, F);
+          const int dst = (K == 0) ? r * EXW + txn : tyn * EXW + r;
+#pragma unroll
+          for (int v = 0; v < NCONS; ++v) S.fx[T.nat[K][v]][dst] = F[v];
+        }
+        bar_work();                                                    // C: fluxes visible
+      }
+    }
+    return;
+  }
+
+  // =================================================================================================
+  // compute warps
+  // =================================================================================================
+  const int tx = tid & (TX - 1), ty = tid / TX;
+  const bool in = tx < txn && ty < tyn;
+  const int base = ty * EXW + tx;                                      // own flux slot = slot of the left state
+  const int hr = lane & 15;                                            // halo unit: row (x) / column (y)
+  const bool hup = lane >= 16;                                         //            lower | upper halo cell
+  long long c = cell_index(G, i0 + tx, j0 + ty, k0 - 2);
+  double* const* Tgt = (STAGE == 1) ? G.Us : G.Un;
+  int st = 0;                                                          // ring stage of the next box to consume
+  unsigned ph = 0;                                                     // and its mbarrier phase parity
+  // k = k0-2: upper-face z states of plane k0-1; k = k0-1: z flux through the lower face of plane k0
+  for (int k = k0 - 2; k < k1; ++k, c += sz) {
+#pragma unroll 1
+    for (int K = (k < k0) ? 2 : 0; K < 3; ++K) {
+      const long long s = G.stride[K];
+      const int up = (K == 0) ? 1 : (K == 1) ? EXW : 0;                // own upper-face slot relative to base
+      const long long cr = (K == 2) ? c + sz : c, cl = cr - s;         // the face this thread solves
+      const bool solve = in && (K < 2 || k >= k0 - 1);
+      // ---- prefetches into registers: face metric; z phase: left states (carry) and the stage target
+      FaceRaw raw;
+      if (solve) load_face_raw(T, K, cl, cr, raw);
+      double PLz[NVR], tgt[NCONS];
+      if (K == 2) {
+#pragma unroll
+        for (int vr = 0; vr < NV; ++vr) PLz[vr] = S.chi[vr][tid];
+        if (in && k >= k0) {
+#pragma unroll
+          for (int v = 0; v < NCONS; ++v) tgt[v] = Tgt[v][c];
+        }
+      }
+      // ---- a2: reconstruction from the staged boxes (own cell: every thread; halo cells: one warp per variable)
+      const int own0 = (K == 0) ? ty * (TX + 6) + tx + 3 : (K == 1) ? (ty + 3) * PY + tx + 1 : (2 * TY + ty) * PY + tx + 1;
+      const int sst = (K == 0) ? 1 : (K == 1) ? PY : PY * TY;
+      const int hal0 = (K == 0) ? hr * (TX + 6) + (hup ? txn + 3 : 2) : (hup ? tyn + 3 : 2) * PY + hr + 1;
+      const bool hvalid = hr < ((K == 0) ? tyn : txn);
+      const bool edge = in && ((K == 0) ? (tx == txn - 1) : (K == 1) ? (ty == tyn - 1) : false);
+      double lo[NVR], cur[5], nxt[5];
+      mbar_wait(&S.full[st], ph);
+      lds_stencil<RECON>(&S.ring[st][own0], sst, cur);
+#pragma unroll
+      for (int vr = 0; vr < NV; ++vr) {
+        const int sn = (st + 1 == NS) ? 0 : st + 1;
+        const unsigned pn = (st + 1 == NS) ? ph ^ 1u : ph;
+        if (vr + 1 < NV) {
+          mbar_wait(&S.full[sn], pn);
+          lds_stencil<RECON>(&S.ring[sn][own0], sst, nxt);
+        }
+        if (K < 2 && warp == vr % NWC) {                               // halo unit of this variable
+          double u[5], l, h;
+          lds_stencil<RECON>(&S.ring[st][hal0], sst, u);
+          recon_cell<RECON>(G.weno_eps, u[0], u[1], u[2], u[3], u[4], l, h);
+          if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
+            if (!(l > 0.0)) l = u[2];
+            if (!(h > 0.0)) h = u[2];
+          }
+          if (hvalid) {
+            if (hup) S.exlo[vr][hr] = l;
+            else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
+          }
+        }
+        double l, h;
+        recon_cell<RECON>(G.weno_eps, cur[0], cur[1], cur[2], cur[3], cur[4], l, h);
+        if (vr < 2) {
+          if (!(l > 0.0)) l = cur[2];
+          if (!(h > 0.0)) h = cur[2];
+        }
+        lo[vr] = l;
+        if (K == 2) S.chi[vr][tid] = h;
+        else {
+          S.ex[vr][base + up] = h;
+          if (edge) S.exhi[vr][(K == 0) ? ty : tx] = h;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&S.empty[st]);
+        st = sn; ph = pn;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) cur[q] = nxt[q];
+      }
+      if (K < 2) bar_work();                                           // A: face states visible
+      // ---- a3: HLLE at the own lower face (x, y) / upper face (z)
+      double F[NCONS];
+      if (solve) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { pin(raw.l[q]); pin(raw.r[q]); }
+        FaceMet m;
+        finish_face_met(raw, m);
+        if (K < 2) {
+#pragma unroll
+          for (int vr = 0; vr < NV; ++vr) PLz[vr] = S.ex[vr][base];
+        }
+        riemann_m<CHARGE, NV>(G, m, cl, cr, PLz, 1, lo, F);
+      }
+      if (K < 2) {
+        if (solve) {
+#pragma unroll
+          for (int v = 0; v < NCONS; ++v) S.fx[T.nat[K][v]][base] = F[v];
+        }
+        bar_work();                                                    // C: fluxes visible
+        if (in) {
+          const double idx = G.inv_dx[K];
+#pragma unroll
+          for (int v = 0; v < NCONS; ++v) S.du[v][tid] -= (S.fx[v][base + up] - S.fx[v][base]) * idx;
+        }
+      } else if (solve) {
+        // z: difference against the flux kept from the previous plane, then a5 (divergence part)
+        const double idz = G.inv_dx[2], w = (STAGE == 1) ? dt : 0.5 * dt;
+        double Fn[NCONS];
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) Fn[nat_z(v)] = F[v] * idz;
+        if (k >= k0) {
+#pragma unroll
+          for (int v = 0; v < NCONS; ++v) {
+            pin(tgt[v]);
+            Tgt[v][c] = tgt[v] + w * (S.du[v][tid] - Fn[v]);
+          }
+        }
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) S.du[v][tid] = Fn[v];          // lower z face of the next plane
+      }
+    }
+  }
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+bool rhs_tma_supported(const GridView& G) {
+  // three active directions; TMA needs 16-byte multiples for every global stride (even row pitch)
+  return G.n[0] > 1 && G.n[1] > 1 && G.n[2] > 1 && (G.stride[1] % 2) == 0 && (G.stride[2] % 2) == 0;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+// Tensor maps over the 17 equally spaced fields P[0..13], jc[0..2] of the slab, viewed as a 4D tensor
+// (x, y, z, field) of doubles; one map per direction (the box shape is part of the map).
+void* tma_create(const GridView& G) {
+  if (!rhs_tma_supported(G)) return nullptr;
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return nullptr;
+  const long long fs = G.P[1] - G.P[0];
+  for (int v = 1; v < NPRIM; ++v) if (G.P[v] - G.P[v - 1] != fs) return nullptr;
+  if (G.jc[0] - G.P[NPRIM - 1] != fs || G.jc[1] - G.jc[0] != fs || G.jc[2] - G.jc[1] != fs) return nullptr;
+  TmaMaps* M = new TmaMaps;
+  const cuuint64_t dims[4] = {(cuuint64_t)G.np[0], (cuuint64_t)G.np[1], (cuuint64_t)G.np[2], (cuuint64_t)(NPRIM + 3)};
+  const cuuint64_t strides[3] = {(cuuint64_t)G.stride[1] * 8, (cuuint64_t)G.stride[2] * 8, (cuuint64_t)fs * 8};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const cuuint32_t boxes[3][4] = {{TX + 6, TY, 1, 1}, {PY, TY + 6, 1, 1}, {PY, TY, 5, 1}};
+  CUtensorMap* maps[3] = {&M->x, &M->y, &M->z};
+  for (int K = 0; K < 3; ++K) {
+    const CUresult r = enc(maps[K], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)G.P[0], dims, strides, boxes[K], estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { delete M; return nullptr; }
+  }
+  return M;
+}
+
+void tma_destroy(void* state) { delete (TmaMaps*)state; }
+
+static int choose_cz(const GridView& G) {
+  // one CTA per SM: pick the pencil length that minimises (waves of 148 CTAs) x (planes per CTA + the two
+  // lead-in z phases, ~2/3 of a plane)
+  const long long tiles = (long long)((G.n[0] + TX - 1) / TX) * ((G.n[1] + TY - 1) / TY);
+  int best = G.n[2];
+  double best_cost = 1e300;
+  for (int chunks = 1; chunks <= G.n[2] && chunks <= 4096; ++chunks) {
+    const int cz = (G.n[2] + chunks - 1) / chunks;
+    if (cz < 4 && chunks > 1) break;
+    const long long ctas = tiles * ((G.n[2] + cz - 1) / cz);
+    const double cost = (double)((ctas + 147) / 148) * (cz + 0.7);
+    if (cost < best_cost) { best_cost = cost; best = cz; }
+  }
+  return best;
+}
+
+template <int RECON, int CHARGE, int STAGE>
+static cudaError_t launch_one(const GridView& G, const TmaMaps& M, double dt, cudaStream_t st) {
+  const int cz = choose_cz(G);
+  const PencilTabs T = make_tabs(G);
+  dim3 block(NTHREADS, 1, 1);
+  dim3 grid((G.n[0] + TX - 1) / TX, (G.n[1] + TY - 1) / TY, (G.n[2] + cz - 1) / cz);
+  const size_t smem = sizeof(Smem);
+  cudaError_t e = cudaFuncSetAttribute(k_flux_tma<RECON, CHARGE, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_flux_tma<RECON, CHARGE, STAGE><<<grid, block, smem, st>>>(G, T, M, dt, cz);
+  return cudaGetLastError();
+}
+
+template <int RECON, int CHARGE>
+static cudaError_t launch_rc(const GridView& G, const TmaMaps& M, double dt, int stage, cudaStream_t st) {
+  return stage == 1 ? launch_one<RECON, CHARGE, 1>(G, M, dt, st) : launch_one<RECON, CHARGE, 2>(G, M, dt, st);
+}
+
+cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int stage, int recon, cudaStream_t st) {
+  if (!state) return cudaErrorInvalidValue;
+  const TmaMaps& M = *(const TmaMaps*)state;
+  const bool ohm = G.charge_mode == CHARGE_FACE_OHM;
+  switch (recon) {
+    case RECON_MINMOD:
+      return ohm ? launch_rc<RECON_MINMOD, CHARGE_FACE_OHM>(G, M, dt, stage, st)
+                 : launch_rc<RECON_MINMOD, CHARGE_CELL_CURRENT>(G, M, dt, stage, st);
+    case RECON_MC:
+      return ohm ? launch_rc<RECON_MC, CHARGE_FACE_OHM>(G, M, dt, stage, st)
+                 : launch_rc<RECON_MC, CHARGE_CELL_CURRENT>(G, M, dt, stage, st);
+    default:
+      return ohm ? launch_rc<RECON_WENO5, CHARGE_FACE_OHM>(G, M, dt, stage, st)
+                 : launch_rc<RECON_WENO5, CHARGE_CELL_CURRENT>(G, M, dt, stage, st);
+  }
+}
+
+}  // namespace rg

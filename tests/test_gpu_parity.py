@@ -51,11 +51,13 @@ def _pair(binding, par, metric, prims, sigma=None, variant=0):
 # random smooth curved periodic problem: every term of the scheme is exercised (shift, K_ij,
 # off-diagonal metric, cleaning fields, charge); ragged sizes that span several tiles + a tail
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("charge_mode", [wl.CHARGE_CELL_CURRENT, wl.CHARGE_FACE_OHM])
 @pytest.mark.parametrize("scheme", [wl.RECON_WENO5, wl.RECON_MC, wl.RECON_MINMOD])
-def test_curved_periodic_block(binding, scheme, charge_mode, variant):
-    n = (37, 11, 9)
+@pytest.mark.parametrize("n", [(38, 21, 9), (37, 11, 9)])
+def test_curved_periodic_block(binding, scheme, charge_mode, variant, n):
+    """(38, 21, 9): even row pitch -> variant 0 is the TMA-staged kernel, tiles 16+16+6 by 16+5; (37, 11, 9): odd
+    pitch -> variant 0 falls back to the pencil kernel (TMA needs 16-byte global strides)."""
     rng = np.random.default_rng(7 + scheme)
     metric, P = _periodic_problem(40, rng, True)
     sl = (slice(None), slice(0, n[2]), slice(0, n[1]), slice(0, n[0]))
@@ -84,7 +86,7 @@ def test_inactive_directions(binding, n3):
     dx = (0.1,) * 3
     for bc in (0, 1):
         par = dict(n=n3, dx=dx, bc=(bc,) * 3, gamma_eos=2.0, sigma_model=0, sigma0=100.0)
-        for variant in (0, 1):
+        for variant in (0, 1, 2):
             g, o = _pair(binding, par, metric, P, variant=variant)
             g.step(0.02, wl.RECON_WENO5); o.step(0.02, wl.RECON_WENO5)
             _compare(g, o, n3, 0.1, TOL1, "n=%s bc=%d variant=%d" % (n3, bc, variant))
@@ -113,7 +115,7 @@ def _run_workload(binding, w, nsteps, fields=None, n=None, bc=None, variant=0, c
     return g, o, worst
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_cfg1_shocktube(binding, variant):
     w = wl.shocktube()
     _run_workload(binding, w, 20, variant=variant)
@@ -131,13 +133,13 @@ def test_cfg1_shocktube_to_t04(binding):
     _compare(g, o, w.n, w.dx[0], 20 * TOL20, "cfg1 t=0.4")
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_cfg2_current_sheet(binding, variant):
     w = wl.current_sheet()
     _run_workload(binding, w, 20, variant=variant)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_cfg3_alfven_reduced(binding, variant):
     w = wl.alfven3d(n=32)
     _run_workload(binding, w, 20, variant=variant)
@@ -147,7 +149,7 @@ def _subblock(w, lo, shape):
     return w.fields(lo, shape), shape, (wl.BC_OUTFLOW,) * 3
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_cfg4_blast_subblock(binding, variant):
     """A 40x36x20 sub-block of the 256^3 grid that contains part of the cylinder edge (outflow
     boundaries on the sub-block: a different problem from the full run, identical on both sides)."""
@@ -156,7 +158,7 @@ def test_cfg4_blast_subblock(binding, variant):
     _run_workload(binding, w, 20, fields=f, n=n, bc=bc, variant=variant)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_cfg5_tov_subblock(binding, variant):
     """A sub-block of the 512^3 grid across the stellar surface (floor resets active)."""
     w = wl.tov_like()
@@ -225,7 +227,7 @@ def test_variants_agree_bitwise_or_to_roundoff(binding):
     w = wl.blast_curved()
     f, n, bc = _subblock(w, (110, 120, 90), (45, 19, 13))
     gs = []
-    for variant in (0, 1):
+    for variant in (0, 1, 2):
         g = binding.from_workload(w, fields=f, n=n, bc=bc)
         g.set_rhs_variant(variant)
         for _ in range(3):
