@@ -14,6 +14,7 @@
 namespace rg {
 cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats, cudaStream_t st);
 cudaError_t launch_prim2cons(const GridView& G, cudaStream_t st);
+cudaError_t launch_metric_coeffs(const GridView& G, cudaStream_t st);
 cudaError_t launch_rhs_simple(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 bool rhs_pencil_supported(const GridView& G);
@@ -144,7 +145,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   G.charge_mode = p->charge_mode;
   G.weno_eps = p->weno_eps > 0.0 ? p->weno_eps : 1e-26;
 
-  const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3;
+  const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3 + rg::NSRC;
   h->field_stride = (G.ntot + 31) / 32 * 32;
   const size_t bytes = (size_t)nfields * (size_t)h->field_stride * sizeof(double);
   cudaError_t e = cudaMalloc((void**)&h->slab, bytes);
@@ -163,6 +164,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   for (int v = 0; v < rg::NCONS; ++v) G.Un[v] = next();
   for (int v = 0; v < rg::NCONS; ++v) G.Us[v] = next();
   for (int v = 0; v < 3; ++v) G.X1[v] = next();
+  for (int v = 0; v < rg::NSRC; ++v) G.src[v] = next();
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(h->slab); cudaFree(h->stats_dev); delete h; return RGRMHD_E_CUDA; }
   h->tma = rg::tma_create(G);
@@ -218,6 +220,8 @@ int rgrmhd_set_metric(rgrmhd_t h, const double* alpha, const double* const beta[
     if ((rc = copy_in(h, h->G.met[rg::MGXX + i], gam[i]))) return rc;
     if ((rc = copy_in(h, h->G.met[rg::MKXX + i], K[i]))) return rc;
   }
+  RG_CUDA(h, rg::launch_metric_coeffs(h->G, h->stream));   // static source coefficients (rgrmhd_sources.cuh)
+  ++h->launches;
   h->have_metric = true;
   return RGRMHD_OK;
 }

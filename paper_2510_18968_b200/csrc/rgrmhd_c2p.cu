@@ -235,9 +235,12 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double al
 //   STAGE 3: recovery of U^{n+1} (G.Un) at fixed calE (a = 0, reading R12); writes P; floor write-back (R9)
 // The guess is the current G.P.  jc = undensitised conduction current of the stage (reading R3).
 constexpr int C2P_TX = 32, C2P_TY = 4;
+#ifndef C2P_MINB
+#define C2P_MINB 3
+#endif
 
 template <int STAGE>
-__global__ void __launch_bounds__(C2P_TX * C2P_TY, 3)
+__global__ void __launch_bounds__(C2P_TX * C2P_TY, C2P_MINB)
 k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stats) {
   const int i = blockIdx.x * C2P_TX + (threadIdx.x & (C2P_TX - 1));
   const int j = blockIdx.y * C2P_TY + (threadIdx.x / C2P_TX);
@@ -295,7 +298,9 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       double S[NCONS];
 #pragma unroll
       for (int v = 0; v < NCONS; ++v) S[v] = 0.0;
-      add_sources(G, c, P, S);
+      Met m;
+      load_met_cell(G, c, m);
+      add_sources(G, c, m, P, S);
       stage_precombine<STAGE>(G, c, dt, S, sgE);
     }
   }
@@ -330,6 +335,28 @@ k_prim2cons(const __grid_constant__ GridView G) {
   prim2cons(m, G.Gamma, P, U);
 #pragma unroll
   for (int v = 0; v < NCONS; ++v) G.Un[v][c] = U[v];
+}
+
+// Static source coefficients of every interior cell (once per set_metric).
+__global__ void __launch_bounds__(128)
+k_metric_coeffs(const __grid_constant__ GridView G) {
+  const int nx = G.n[0], ny = G.n[1];
+  const long long nint = (long long)nx * ny * G.n[2];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nint) return;
+  const int i = (int)(t % nx);
+  const long long r = t / nx;
+  const long long c = cell_index(G, i, (int)(r % ny), (int)(r / ny));
+  double out[NSRC];
+  metric_coeffs_cell(G, c, out);
+#pragma unroll
+  for (int q = 0; q < NSRC; ++q) G.src[q][c] = out[q];
+}
+
+cudaError_t launch_metric_coeffs(const GridView& G, cudaStream_t st) {
+  const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
+  k_metric_coeffs<<<(unsigned)((nint + 127) / 128), 128, 0, st>>>(G);
+  return cudaGetLastError();
 }
 
 // ---- launchers -----------------------------------------------------------------------------------

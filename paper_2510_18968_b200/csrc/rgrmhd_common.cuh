@@ -14,7 +14,7 @@
 
 namespace rg {
 
-enum { NPRIM = 14, NCONS = 14, NMET = 16 };
+enum { NPRIM = 14, NCONS = 14, NMET = 16, NSRC = 34 };
 // primitive indices
 enum { RHO = 0, PRS, VX, VY, VZ, EX, EY, EZ, BX, BY, BZ, PSI, PHI, QCH };
 // conserved indices
@@ -44,6 +44,7 @@ struct GridView {
   double* Un[NCONS];     // U^n, overwritten with U^{n+1} by the stage-2 combine
   double* Us[NCONS];     // stage vector U*^(2)
   double* X1[3];         // calE^(1) (needed again by the final combine, Eq. 37)
+  double* src[NSRC];     // static source coefficients (metric derivatives, G^i, tr K; rgrmhd_sources.cuh)
 };
 
 struct StatsDev {

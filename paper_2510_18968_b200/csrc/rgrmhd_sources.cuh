@@ -12,18 +12,74 @@ __device__ __forceinline__ double d4(const double* __restrict__ f, long long c, 
   return (-__ldg(f + c + 2 * s) + 8.0 * __ldg(f + c + s) - 8.0 * __ldg(f + c - s) + __ldg(f + c - 2 * s)) * inv_12dx;
 }
 
+// Static source coefficients.  The metric is fixed in time (north_star), so everything in the sources that
+// depends on the metric alone is computed ONCE per set_metric (k_metric_coeffs) and stored as NSRC fields:
+//   SRC_DAL + d          d_d alpha                       (3)
+//   SRC_DB  + 3 d + a    d_d beta^a                      (9)
+//   SRC_DG  + 6 d + q    d_d gamma_q, q = xx..zz         (18)
+//   SRC_GA  + a          G^a = gamma^ab d_b alpha - alpha gamma^al gamma^jk (d_j gamma_lk - 1/2 d_l gamma_jk)   (3)
+//   SRC_TRK              K = gamma^ij K_ij               (1)
+// with the 4th-order centred differences of reading R2 (inactive direction -> 0).
+enum { SRC_DAL = 0, SRC_DB = 3, SRC_DG = 12, SRC_GA = 30, SRC_TRK = 33 };
+static_assert(SRC_TRK + 1 == NSRC, "source coefficient count");
+
+__device__ __forceinline__ void metric_coeffs_cell(const GridView& G, long long c, double out[NSRC]) {
+  Met m;
+  load_met_cell(G, c, m);
+  double trK = 0.0;
+#pragma unroll
+  for (int q = 0; q < 6; ++q)
+    trK += ((q == 0 || q == 3 || q == 5) ? 1.0 : 2.0) * m.gi[q] * __ldg(G.met[MKXX + q] + c);
+  out[SRC_TRK] = trK;
+  double Cl[3] = {0.0, 0.0, 0.0}, da[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    double dal = 0.0, db[3] = {0.0, 0.0, 0.0}, dg[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if (G.n[d] > 1) {
+      const long long s = G.stride[d];
+      const double w = G.inv_12dx[d];
+      dal = d4(G.met[MALP], c, s, w);
+#pragma unroll
+      for (int a = 0; a < 3; ++a) db[a] = d4(G.met[MBX + a], c, s, w);
+#pragma unroll
+      for (int q = 0; q < 6; ++q) dg[q] = d4(G.met[MGXX + q], c, s, w);
+    }
+    da[d] = dal;
+    double gdg = 0.0;
+#pragma unroll
+    for (int q = 0; q < 6; ++q) gdg += ((q == 0 || q == 3 || q == 5) ? 1.0 : 2.0) * m.gi[q] * dg[q];
+#pragma unroll
+    for (int l = 0; l < 3; ++l)
+      Cl[l] += m.gi[sym(d, 0)] * dg[sym(l, 0)] + m.gi[sym(d, 1)] * dg[sym(l, 1)] + m.gi[sym(d, 2)] * dg[sym(l, 2)];
+    Cl[d] -= 0.5 * gdg;
+    out[SRC_DAL + d] = dal;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) out[SRC_DB + 3 * d + a] = db[a];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) out[SRC_DG + 6 * d + q] = dg[q];
+  }
+  double Gi[3], gda[3];
+  raise(m, Cl, Gi);
+  raise(m, da, gda);
+#pragma unroll
+  for (int a = 0; a < 3; ++a) out[SRC_GA + a] = gda[a] - m.alpha * Gi[a];
+}
+
 // a4 (second half). explicit sources at a cell centre (Eq. 27 S; Eq. 39-40;
-// reading R1 / SURVEY.md O6).  P = the cell's primitives; ADDS the sources to S[].
+// reading R1 / SURVEY.md O6).  P = the cell's primitives, m = the cell's metric; ADDS the sources to S[].
 //   S(S_i)  = 1/2 alpha sg T^jk d_i gamma_jk + S_j d_i beta^j - (tau + D) d_i alpha
 //   S(tau)  = alpha sg T^ij K_ij - S^j d_j alpha
 //   S(calB^i) = -calB^k d_k beta^i + Phi G^i ;  S(calE^i) = -calE^k d_k beta^i + Psi G^i - alpha calQ v^i
 //   S(Phi)  = -alpha Phi K + calB^k d_k alpha - alpha kappa Phi ;  S(Psi) likewise + alpha calQ
-//   G^i = gamma^ij d_j alpha - alpha gamma^il gamma^jk (d_j gamma_lk - 1/2 d_l gamma_jk)
-// The metric derivatives (4th-order centred, reading R2) are consumed direction by direction so that
-// only one direction's ten derivatives are live at a time.
-__device__ __forceinline__ void add_sources(const GridView& G, long long c, const double P[NPRIM], double S[NCONS]) {
-  Met m;
-  load_met_cell(G, c, m);
+// All metric derivatives, G^i and K come from the static coefficient fields (G.src): 40 coalesced loads,
+// no stencil.
+__device__ __forceinline__ void add_sources(const GridView& G, long long c, const Met& m, const double P[NPRIM],
+                                            double S[NCONS]) {
+  double src[NSRC], Kq[6];
+#pragma unroll
+  for (int q = 0; q < NSRC; ++q) src[q] = __ldg(G.src[q] + c);
+#pragma unroll
+  for (int q = 0; q < 6; ++q) Kq[q] = __ldg(G.met[MKXX + q] + c);
   const double rho = P[RHO], p = P[PRS];
   const double vU[3] = {P[VX], P[VY], P[VZ]}, EU[3] = {P[EX], P[EY], P[EZ]}, BU[3] = {P[BX], P[BY], P[BZ]};
   double vD[3], ED[3], BD[3], ExB[3];
@@ -52,57 +108,34 @@ __device__ __forceinline__ void add_sources(const GridView& G, long long c, cons
   const double cE[3] = {sg * EU[0], sg * EU[1], sg * EU[2]}, cB[3] = {sg * BU[0], sg * BU[1], sg * BU[2]};
   const double cPsi = sg * P[PSI], cPhi = sg * P[PHI], cQ = sg * P[QCH];
   const double asg = al * sg;
-  double trK = 0.0;
   {
     double t1 = 0.0;
 #pragma unroll
-    for (int q = 0; q < 6; ++q) {
-      const double Kq = __ldg(G.met[MKXX + q] + c);
-      t1 += Tw[q] * Kq;
-      trK += ((q == 0 || q == 3 || q == 5) ? 1.0 : 2.0) * m.gi[q] * Kq;
-    }
+    for (int q = 0; q < 6; ++q) t1 += Tw[q] * Kq[q];
     S[CTAU] += asg * t1;
   }
-  double Cl[3] = {0.0, 0.0, 0.0}, da[3] = {0.0, 0.0, 0.0};
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    if (G.n[d] > 1) {
-      const long long s = G.stride[d];
-      const double w = G.inv_12dx[d];
-      const double dal = d4(G.met[MALP], c, s, w);
-      double db[3], dg[6];
+    const double dal = src[SRC_DAL + d];
+    const double* db = &src[SRC_DB + 3 * d];
+    const double* dg = &src[SRC_DG + 6 * d];
+    double tg = 0.0;
 #pragma unroll
-      for (int a = 0; a < 3; ++a) db[a] = d4(G.met[MBX + a], c, s, w);
+    for (int q = 0; q < 6; ++q) tg += Tw[q] * dg[q];
+    S[CSX + d] += 0.5 * asg * tg + (SD[0] * db[0] + SD[1] * db[1] + SD[2] * db[2]) - tauD * dal;
+    S[CTAU] -= SU[d] * dal;
 #pragma unroll
-      for (int q = 0; q < 6; ++q) dg[q] = d4(G.met[MGXX + q], c, s, w);
-      da[d] = dal;
-      double tg = 0.0, gdg = 0.0;
-#pragma unroll
-      for (int q = 0; q < 6; ++q) {
-        tg += Tw[q] * dg[q];
-        gdg += ((q == 0 || q == 3 || q == 5) ? 1.0 : 2.0) * m.gi[q] * dg[q];
-      }
-      S[CSX + d] += 0.5 * asg * tg + (SD[0] * db[0] + SD[1] * db[1] + SD[2] * db[2]) - tauD * dal;
-      S[CTAU] -= SU[d] * dal;
-#pragma unroll
-      for (int l = 0; l < 3; ++l)
-        Cl[l] += m.gi[sym(d, 0)] * dg[sym(l, 0)] + m.gi[sym(d, 1)] * dg[sym(l, 1)] + m.gi[sym(d, 2)] * dg[sym(l, 2)];
-      Cl[d] -= 0.5 * gdg;
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        S[CBX + a] -= cB[d] * db[a];
-        S[CEX + a] -= cE[d] * db[a];
-      }
-      S[CPHI] += cB[d] * dal;
-      S[CPSI] += cE[d] * dal;
+    for (int a = 0; a < 3; ++a) {
+      S[CBX + a] -= cB[d] * db[a];
+      S[CEX + a] -= cE[d] * db[a];
     }
+    S[CPHI] += cB[d] * dal;
+    S[CPSI] += cE[d] * dal;
   }
-  double Gi[3], gda[3];
-  raise(m, Cl, Gi);
-  raise(m, da, gda);
+  const double trK = src[SRC_TRK];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    const double Ga = gda[a] - al * Gi[a];
+    const double Ga = src[SRC_GA + a];
     S[CBX + a] += cPhi * Ga;
     S[CEX + a] += cPsi * Ga - al * cQ * vU[a];
   }
