@@ -31,7 +31,7 @@ constexpr int TX = 16, TY = 16, NT = TX * TY;
 constexpr int NWC = NT / 32;                       // compute warps
 constexpr int NTHREADS = NT + 64;                  // + producer warp + edge-face warp
 constexpr int EXW = TX + 1, EXH = TY + 1, EXP = EXW * EXH;
-constexpr int NS = 6;                              // ring stages
+constexpr int NS = 5;                              // ring stages
 // The TMA engine needs a 16-byte aligned box origin (an even x coordinate for doubles: an odd one traps with
 // "illegal instruction"), and the ghost offset is 3: the y and z boxes therefore start one cell left of the tile
 // and are TX + 2 wide.
@@ -47,7 +47,7 @@ struct Smem {
   double fx[NCONS][EXP];        // face fluxes (slot = the cell whose lower face it is; column TX / row TY = edge)
   double exlo[NVR][16];         // lower-face states of the upper-halo cells (right states of the edge faces)
   double exhi[NVR][16];         // upper-face states of the last row/column (left states of the edge faces)
-  double chi[NVR][NT];          // z carry: upper-face states of the current plane
+  double chi[2][NVR][NT];       // z carry: upper-face states of the plane below / being reconstructed (by parity of k)
   double du[NCONS][NT];         // flux divergence being accumulated for the current plane (thread-private)
   unsigned long long full[NS], empty[NS];
 };
@@ -72,6 +72,31 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
       "bra W_%=;\n"
       "D_%=:\n"
       "}\n" ::"r"(a), "r"(parity) : "memory");
+}
+// one non-blocking probe: issue early, test the result later (the probe's ~90-cycle latency hides behind
+// independent arithmetic)
+__device__ __forceinline__ unsigned mbar_test(unsigned long long* b, unsigned parity) {
+  unsigned ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n" : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+  return ok;
+}
+// producer-side wait: long hardware suspend per probe, so the spinning lane does not take issue slots
+__device__ __forceinline__ void mbar_wait_sleepy(unsigned long long* b, unsigned parity) {
+  const unsigned a = smem_u32(b);
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "W_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+      "@p bra D_%=;\n"
+      "bra W_%=;\n"
+      "D_%=:\n"
+      "}\n" ::"r"(a), "r"(parity), "r"(100000u) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
@@ -105,6 +130,7 @@ __device__ __forceinline__ void lds_stencil(const double* __restrict__ p, int s,
 }  // namespace
 
 template <int RECON, int CHARGE, int STAGE>
+// 168 registers: 10 warps sit 3 + 3 + 2 + 2 on the four schedulers, each with a 16 K-register file
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTabs T,
            const __grid_constant__ TmaMaps M, double dt, int CZ) {
@@ -140,7 +166,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           const int px = i0 + ((K == 0) ? 0 : 2), py = j0 + ((K == 1) ? 0 : 3), pz = k + ((K == 2) ? 2 : 3);
           for (int vr = 0; vr < NV; ++vr, ++seq) {
             const int st = seq % NS, it = seq / NS;
-            if (it > 0) mbar_wait(&S.empty[st], (unsigned)(it - 1) & 1u);
+            if (it > 0) mbar_wait_sleepy(&S.empty[st], (unsigned)(it - 1) & 1u);
             mbar_expect_tx(&S.full[st], bytes);
             tma_load_4d(map, S.ring[st], &S.full[st], px, py, pz, T.fld[K][vr]);
           }
@@ -202,65 +228,105 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
       const int up = (K == 0) ? 1 : (K == 1) ? EXW : 0;                // own upper-face slot relative to base
       const long long cr = (K == 2) ? c + sz : c, cl = cr - s;         // the face this thread solves
       const bool solve = in && (K < 2 || k >= k0 - 1);
-      // ---- prefetches into registers: face metric; z phase: left states (carry) and the stage target
-      FaceRaw raw;
-      if (solve) load_face_raw(T, K, cl, cr, raw);
-      double PLz[NVR], tgt[NCONS];
-      if (K == 2) {
-#pragma unroll
-        for (int vr = 0; vr < NV; ++vr) PLz[vr] = S.chi[vr][tid];
-        if (in && k >= k0) {
-#pragma unroll
-          for (int v = 0; v < NCONS; ++v) tgt[v] = Tgt[v][c];
-        }
-      }
-      // ---- a2: reconstruction from the staged boxes (own cell: every thread; halo cells: one warp per variable)
+      // ---- a2: reconstruction from the staged boxes, two variables per step so that two independent
+      // dependency chains interleave.  fetch(pair): wait for the pair's boxes, read the own stencils into
+      // registers, let the pair's halo warp reconstruct the tile's halo cells straight away, and hand the
+      // stages back to the producer -- one step BEFORE the own cells of that pair are reconstructed.
       const int own0 = (K == 0) ? ty * (TX + 6) + tx + 3 : (K == 1) ? (ty + 3) * PY + tx + 1 : (2 * TY + ty) * PY + tx + 1;
       const int sst = (K == 0) ? 1 : (K == 1) ? PY : PY * TY;
       const int hal0 = (K == 0) ? hr * (TX + 6) + (hup ? txn + 3 : 2) : (hup ? tyn + 3 : 2) * PY + hr + 1;
       const bool hvalid = hr < ((K == 0) ? tyn : txn);
       const bool edge = in && ((K == 0) ? (tx == txn - 1) : (K == 1) ? (ty == tyn - 1) : false);
-      double lo[NVR], cur[5], nxt[5];
-      mbar_wait(&S.full[st], ph);
-      lds_stencil<RECON>(&S.ring[st][own0], sst, cur);
+      double* const hi_dst = (K == 2) ? &S.chi[(k & 1)][0][tid] : &S.ex[0][base + up];
+      const int hi_str = (K == 2) ? NT : EXP;
+      FaceRaw raw;
+      double lo[NVR], cur[2][5], nxt[2][5];
+      unsigned rdy0 = 0, rdy1 = 0;                                     // probe results for the next pair's boxes
+      auto fetch = [&](int v0, double (&dst)[2][5], unsigned r0, unsigned r1) {
+        const int s0 = st;
+        const unsigned p0 = ph;
+        const int s1 = (s0 + 1 == NS) ? 0 : s0 + 1;
+        const unsigned p1 = (s0 + 1 == NS) ? p0 ^ 1u : p0;
+        const bool two = v0 + 1 < NV;
+        const bool howner = K < 2 && warp == (v0 >> 1) % NWC;
+        double u[2][5];
+        if (!r0) mbar_wait(&S.full[s0], p0);
+        lds_stencil<RECON>(&S.ring[s0][own0], sst, dst[0]);
+        if (howner) lds_stencil<RECON>(&S.ring[s0][hal0], sst, u[0]);
+        if (two) {
+          if (!r1) mbar_wait(&S.full[s1], p1);
+          lds_stencil<RECON>(&S.ring[s1][own0], sst, dst[1]);
+          if (howner) lds_stencil<RECON>(&S.ring[s1][hal0], sst, u[1]);
+        }
+        if (howner) {                                                  // halo cells of this pair (x, y only)
 #pragma unroll
-      for (int vr = 0; vr < NV; ++vr) {
-        const int sn = (st + 1 == NS) ? 0 : st + 1;
-        const unsigned pn = (st + 1 == NS) ? ph ^ 1u : ph;
-        if (vr + 1 < NV) {
-          mbar_wait(&S.full[sn], pn);
-          lds_stencil<RECON>(&S.ring[sn][own0], sst, nxt);
-        }
-        if (K < 2 && warp == vr % NWC) {                               // halo unit of this variable
-          double u[5], l, h;
-          lds_stencil<RECON>(&S.ring[st][hal0], sst, u);
-          recon_cell<RECON>(G.weno_eps, u[0], u[1], u[2], u[3], u[4], l, h);
-          if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
-            if (!(l > 0.0)) l = u[2];
-            if (!(h > 0.0)) h = u[2];
+          for (int j = 0; j < 2; ++j) {
+            if (j == 0 || two) {
+              const int vr = v0 + j;
+              double l, h;
+              recon_cell<RECON>(G.weno_eps, u[j][0], u[j][1], u[j][2], u[j][3], u[j][4], l, h);
+              if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
+                if (!(l > 0.0)) l = u[j][2];
+                if (!(h > 0.0)) h = u[j][2];
+              }
+              if (hvalid) {
+                if (hup) S.exlo[vr][hr] = l;
+                else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
+              }
+            }
           }
-          if (hvalid) {
-            if (hup) S.exlo[vr][hr] = l;
-            else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
-          }
-        }
-        double l, h;
-        recon_cell<RECON>(G.weno_eps, cur[0], cur[1], cur[2], cur[3], cur[4], l, h);
-        if (vr < 2) {
-          if (!(l > 0.0)) l = cur[2];
-          if (!(h > 0.0)) h = cur[2];
-        }
-        lo[vr] = l;
-        if (K == 2) S.chi[vr][tid] = h;
-        else {
-          S.ex[vr][base + up] = h;
-          if (edge) S.exhi[vr][(K == 0) ? ty : tx] = h;
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&S.empty[st]);
-        st = sn; ph = pn;
+        if (lane == 0) {
+          mbar_arrive(&S.empty[s0]);
+          if (two) mbar_arrive(&S.empty[s1]);
+        }
+        st = two ? ((s1 + 1 == NS) ? 0 : s1 + 1) : s1;
+        ph = two ? ((s1 + 1 == NS) ? p1 ^ 1u : p1) : p1;
+      };
+      auto probe = [&](int v0) {                                       // non-blocking probes of the pair at (st, ph)
+        rdy0 = mbar_test(&S.full[st], ph);
+        rdy1 = 0;
+        if (v0 + 1 < NV) {
+          const int s1 = (st + 1 == NS) ? 0 : st + 1;
+          rdy1 = mbar_test(&S.full[s1], (st + 1 == NS) ? ph ^ 1u : ph);
+        }
+      };
+      fetch(0, cur, 0u, 0u);
+      if (2 < NV) probe(2);
+      constexpr int VRAW = (((NV + 1) / 2 > 3) ? (NV + 1) / 2 - 3 : 0) * 2;   // pair at which the face metric is fetched
 #pragma unroll
-        for (int q = 0; q < 5; ++q) cur[q] = nxt[q];
+      for (int v = 0; v < NV; v += 2) {
+        if (v + 2 < NV) {
+          fetch(v + 2, nxt, rdy0, rdy1);
+          if (v + 4 < NV) probe(v + 4);
+        }
+        if (v == VRAW && solve) load_face_raw(T, K, cl, cr, raw);     // consumed after the loop
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          if (v + j < NV) {
+            const int vr = v + j;
+            double l, h;
+            recon_cell<RECON>(G.weno_eps, cur[j][0], cur[j][1], cur[j][2], cur[j][3], cur[j][4], l, h);
+            if (vr < 2) {
+              if (!(l > 0.0)) l = cur[j][2];
+              if (!(h > 0.0)) h = cur[j][2];
+            }
+            lo[vr] = l;
+            hi_dst[vr * hi_str] = h;
+            if (edge) S.exhi[vr][(K == 0) ? ty : tx] = h;
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j)
+#pragma unroll
+          for (int q = 0; q < 5; ++q) cur[j][q] = nxt[j][q];
+      }
+      // ---- prefetch of the stage target (z phase), consumed after the Riemann solve
+      double PLz[NVR], tgt[NCONS];
+      if (K == 2 && in && k >= k0) {
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) tgt[v] = Tgt[v][c];
       }
       if (K < 2) bar_work();                                           // A: face states visible
       // ---- a3: HLLE at the own lower face (x, y) / upper face (z)
@@ -270,9 +336,11 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         for (int q = 0; q < 8; ++q) { pin(raw.l[q]); pin(raw.r[q]); }
         FaceMet m;
         finish_face_met(raw, m);
-        if (K < 2) {
+        {
+          const double* pl = (K == 2) ? &S.chi[(k & 1) ^ 1][0][tid] : &S.ex[0][base];
+          const int pls = (K == 2) ? NT : EXP;
 #pragma unroll
-          for (int vr = 0; vr < NV; ++vr) PLz[vr] = S.ex[vr][base];
+          for (int vr = 0; vr < NV; ++vr) PLz[vr] = pl[vr * pls];
         }
         riemann_m<CHARGE, NV>(G, m, cl, cr, PLz, 1, lo, F);
       }
