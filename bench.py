@@ -9,8 +9,8 @@ a6) over the workload.  Inputs are seeded and synthetic (paper_2510_18968_b200/w
 * ``value``     zone-cycles/s with the state resident in HBM (whole job: all ranks' zones / max time)
 * ``e2e``       the same metric through the C-ABI with HOST buffers: every step uploads the primitives
                 from pinned host memory (set_prims), steps, and reads the primitives back (get_prims)
-* ``roofline``  the dominant kernel (the fused RHS kernel) against the measured FP64 DFMA peak or the
-                measured HBM copy bandwidth, whichever bounds it
+* ``roofline``  the dominant kernel (the TMA-staged flux-divergence kernel) against the measured FP64 DFMA
+                peak or the measured HBM copy bandwidth, whichever bounds it
 * ``cpu_baseline``  the CPU oracle, as it stands (single thread), on a bounded sample of the same workload
 
 ``--impl reference`` times the oracle instead (the paper ships no code; the oracle is the reference arm).
@@ -38,10 +38,13 @@ from paper_2510_18968_b200 import workloads as wl  # noqa: E402
 METRIC = "zone-cycles/sec per IMEX-RK2 step (FP64)"
 UNIT = "zone-cycles/s"
 
-# Algorithmic work of the dominant kernel (fused reconstruct + HLLE + divergence + sources + combine),
-# per interior cell and launch -- derivation in DESIGN.md Sec. 7.
-RHS_FLOPS = {wl.RECON_WENO5: 6800.0, wl.RECON_MC: 3100.0, wl.RECON_MINMOD: 2900.0}
-RHS_DOUBLES = 69.5      # (61 + 78)/2: stage 1 reads P14 jc3 metric16 Un14, writes Us14; stage 2 adds Us14, X1 3
+# Algorithmic work of the dominant kernel (flux divergence: reconstruct + HLLE + divergence + update of the
+# stage target), per interior cell and launch -- derivation in DESIGN.md Sec. 7.
+RHS_FLOPS = {wl.RECON_WENO5: 5500.0, wl.RECON_MC: 1900.0, wl.RECON_MINMOD: 1800.0}
+RHS_DOUBLES = 55.0      # reads P 14 + jc 3 + alpha, beta, gamma_ij 10 + stage target 14, writes stage target 14
+SRC_FLOPS = 350.0       # explicit sources + point-wise stage combine (inside the recovery kernel), per stage
+C2P_SETUP_FLOPS, C2P_EVAL_FLOPS = 250.0, 100.0   # per solve / per residual evaluation
+STEP_DOUBLES = 253.0    # algorithmic traffic of one zone-cycle
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz = 37.2
 
 
@@ -157,6 +160,49 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------------------
+# rank plumbing ("replicas only": the path does not shard, so the only cross-rank operations are the
+# barrier around the timed region and the max of the per-rank times)
+# ----------------------------------------------------------------------------------------------
+class Ranks:
+    """torch.distributed wrapper used by bench.py: NCCL on the GPU box, gloo in the CPU test."""
+
+    def __init__(self, world: int, backend: str, local: int = 0):
+        self.world, self.backend, self.dist = world, backend, None
+        if world > 1:
+            import torch
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            if backend == "nccl":
+                dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+            else:
+                dist.init_process_group(backend)
+            self.dist = dist
+
+    def barrier(self):
+        import torch
+        if self.dist is not None:
+            self.dist.barrier()
+        if self.backend == "nccl":
+            torch.cuda.synchronize()
+
+    def max_over_ranks(self, x: float) -> float:
+        if self.dist is None:
+            return x
+        import torch
+        t = torch.tensor([x], dtype=torch.float64, device="cuda" if self.backend == "nccl" else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def aggregate(self, units_per_rank: int, steps: int, ms_local: float) -> float:
+        """Whole-job throughput: units all ranks processed / max-over-ranks time."""
+        return self.world * units_per_rank * steps / (self.max_over_ranks(ms_local) * 1e-3)
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
+# ----------------------------------------------------------------------------------------------
 # the CUDA path
 # ----------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -169,23 +215,9 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    ranks = Ranks(world, "nccl", local)
+    barrier, max_over_ranks = ranks.barrier, ranks.max_over_ranks
+    dist = ranks.dist
 
     w = get_workload(args.config)
     f = w.fields()                                     # every replica: the same seeded workload
@@ -264,7 +296,7 @@ def run_ours(args):
                 "peak_kind": "%s copy bandwidth (MEASURED_PEAKS.json)" % peak_kind}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["traffic"] = None
-    roof["kernel"] = "k_rhs_tiled" if args.rhs_variant == 0 else "k_rhs_simple"
+    roof["kernel"] = {0: "k_flux_tma", 1: "k_rhs_simple", 2: "k_rhs_pencil"}[args.rhs_variant]
     roof["avg_launch_ms"] = rhs_avg_s * 1e3
     roof["alg_flops_per_cell"] = RHS_FLOPS[w.recon]
     roof["alg_bytes_per_cell"] = RHS_DOUBLES * 8.0
@@ -274,8 +306,9 @@ def run_ours(args):
     roof["share_of_step"] = shares["rhs"]
     # whole-step roofline (north_star: the slower of bytes at HBM bandwidth and FP64 flops at peak)
     evals_per_solve = stats["c2p_evals"] / max(stats["c2p_solves"], 1)
-    step_flops = 2 * RHS_FLOPS[w.recon] + 3 * 250.0 + 3 * evals_per_solve * 110.0
-    step_bytes = 253 * 8.0
+    step_flops = (2 * RHS_FLOPS[w.recon] + 2 * SRC_FLOPS + 3 * C2P_SETUP_FLOPS +
+                  3 * evals_per_solve * C2P_EVAL_FLOPS)
+    step_bytes = STEP_DOUBLES * 8.0
     t_step_roof = max(step_flops / (fp64_peak * 1e12), step_bytes / (hbm_gbs * 1e9))
     step_roof = {"zone_cycles_per_s_at_roofline": 1.0 / t_step_roof, "frac": value / world * t_step_roof,
                  "flops_per_zone_cycle": step_flops, "bytes_per_zone_cycle": step_bytes,

@@ -107,7 +107,9 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double al
   double Z = (P[RHO] + Gamma / (Gamma - 1.0) * P[PRS]) * W * W;
   bool converged = false, state_ok = false;
   const int max_outer = 50;
-  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, islope = 1.0;
+  // inverse slope of g for the first secant step: dg/dZ ~ 1 - (Gamma-1)/Gamma / W^2 at fixed v (exact in the
+  // unmagnetised, slow limit), instead of 1
+  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, islope = 1.0 / (1.0 - gm1og * (1.0 - v2g));
   // frozen per outer pass
   double s = 0, r = 0, i1s = 1, Npar[3] = {0, 0, 0}, Nperp[3] = {0, 0, 0}, BxN[3] = {0, 0, 0};
   // last evaluation
@@ -235,6 +237,12 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double al
 //   STAGE 3: recovery of U^{n+1} (G.Un) at fixed calE (a = 0, reading R12); writes P; floor write-back (R9)
 // The guess is the current G.P.  jc = undensitised conduction current of the stage (reading R3).
 constexpr int C2P_TX = 32, C2P_TY = 4;
+// staging slots of the point-wise right-hand side (doubles per thread)
+enum { PF_SRC = 0, PF_K = NSRC, PF_UN = NSRC + 6, PF_X1 = NSRC + 6 + NCONS, PF_COUNT = NSRC + 6 + NCONS + 3 };
+__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src)
+               : "memory");
+}
 #ifndef C2P_MINB
 #define C2P_MINB 3
 #endif
@@ -264,6 +272,25 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
 #pragma unroll
     for (int v = 0; v < 5; ++v) P[v] = G.P[v][c];
     const double sigma = (STAGE == 3) ? 0.0 : sigma_of(G, U[CD] / sg, c);
+    // The point-wise right-hand side after the solve reads ~57 more fields of this cell.  Start those loads
+    // now as asynchronous copies into a thread-private shared-memory column: no registers are held and
+    // the solve below hides their DRAM latency.
+    extern __shared__ double pf_smem[];
+    double* const pf = pf_smem + threadIdx.x;              // pf[q * NTH]: conflict-free, private to this thread
+    constexpr int NTH = C2P_TX * C2P_TY;
+    if (STAGE != 3) {
+#pragma unroll
+      for (int q = 0; q < NSRC; ++q) cp_async8(pf + (PF_SRC + q) * NTH, G.src[q] + c);
+#pragma unroll
+      for (int q = 0; q < 6; ++q) cp_async8(pf + (PF_K + q) * NTH, G.met[MKXX + q] + c);
+#pragma unroll
+      for (int v = 0; v < NCONS; ++v) cp_async8(pf + (PF_UN + v) * NTH, G.Un[v] + c);
+      if (STAGE == 2) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) cp_async8(pf + (PF_X1 + q) * NTH, G.X1[q] + c);
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    }
     C2POut r2 = c2p_solve(t, sg, alpha, G.Gamma, U, adt, sigma, G.tol, G.maxit, P);
     evals = r2.evals; failed = r2.failed;
     if (G.rho_floor > 0.0 && (r2.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
@@ -300,8 +327,20 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       for (int v = 0; v < NCONS; ++v) S[v] = 0.0;
       Met m;
       load_met_cell(G, c, m);
-      add_sources(G, c, m, P, S);
-      stage_precombine<STAGE>(G, c, dt, S, sgE);
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      double src[NSRC], Kq[6], un[NCONS], x1[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+      for (int q = 0; q < NSRC; ++q) src[q] = pf[(PF_SRC + q) * NTH];
+#pragma unroll
+      for (int q = 0; q < 6; ++q) Kq[q] = pf[(PF_K + q) * NTH];
+      add_sources(G, m, src, Kq, P, S);
+#pragma unroll
+      for (int v = 0; v < NCONS; ++v) un[v] = pf[(PF_UN + v) * NTH];
+      if (STAGE == 2) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) x1[q] = pf[(PF_X1 + q) * NTH];
+      }
+      stage_precombine<STAGE>(G, c, dt, S, sgE, un, x1);
     }
   }
   // stats: warp reduce, one atomic per warp
@@ -364,9 +403,17 @@ cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats,
   const dim3 block(C2P_TX * C2P_TY, 1, 1);
   const dim3 grid((G.n[0] + C2P_TX - 1) / C2P_TX, (G.n[1] + C2P_TY - 1) / C2P_TY, G.n[2]);
   if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
-  if (stage == 1) k_c2p<1><<<grid, block, 0, st>>>(G, dt, stats);
-  else if (stage == 2) k_c2p<2><<<grid, block, 0, st>>>(G, dt, stats);
-  else k_c2p<3><<<grid, block, 0, st>>>(G, dt, stats);
+  const size_t smem = (size_t)PF_COUNT * C2P_TX * C2P_TY * sizeof(double);
+  cudaError_t e;
+  if (stage == 1) {
+    if ((e = cudaFuncSetAttribute(k_c2p<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    k_c2p<1><<<grid, block, smem, st>>>(G, dt, stats);
+  } else if (stage == 2) {
+    if ((e = cudaFuncSetAttribute(k_c2p<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    k_c2p<2><<<grid, block, smem, st>>>(G, dt, stats);
+  } else {
+    k_c2p<3><<<grid, block, 0, st>>>(G, dt, stats);
+  }
   return cudaGetLastError();
 }
 

@@ -73,13 +73,9 @@ __device__ __forceinline__ void metric_coeffs_cell(const GridView& G, long long 
 //   S(Phi)  = -alpha Phi K + calB^k d_k alpha - alpha kappa Phi ;  S(Psi) likewise + alpha calQ
 // All metric derivatives, G^i and K come from the static coefficient fields (G.src): 40 coalesced loads,
 // no stencil.
-__device__ __forceinline__ void add_sources(const GridView& G, long long c, const Met& m, const double P[NPRIM],
-                                            double S[NCONS]) {
-  double src[NSRC], Kq[6];
-#pragma unroll
-  for (int q = 0; q < NSRC; ++q) src[q] = __ldg(G.src[q] + c);
-#pragma unroll
-  for (int q = 0; q < 6; ++q) Kq[q] = __ldg(G.met[MKXX + q] + c);
+// src[NSRC], Kq[6]: the cell's static coefficients and K_ij (the caller stages them, rgrmhd_c2p.cu).
+__device__ __forceinline__ void add_sources(const GridView& G, const Met& m, const double src[NSRC], const double Kq[6],
+                                            const double P[NPRIM], double S[NCONS]) {
   const double rho = P[RHO], p = P[PRS];
   const double vU[3] = {P[VX], P[VY], P[VZ]}, EU[3] = {P[EX], P[EY], P[EZ]}, BU[3] = {P[BX], P[BY], P[BZ]};
   double vD[3], ED[3], BD[3], ExB[3];
@@ -149,18 +145,17 @@ __device__ __forceinline__ void add_sources(const GridView& G, long long c, cons
 //   STAGE 1:  U*2     = [U^n + dt S1 + (1-2 gamma)/gamma (X1 - X^n)|_X]                        - dt div F1
 //   STAGE 2:  U^{n+1} = [(U^n + U*2)/2 + dt/2 S2 + ((X1 - X^n) + (X2 - X*2)/(2 gamma))|_X]   - dt/2 div F2
 // (dt F1 is carried by U*2).  This function writes the bracket: stage 1 into G.Us, stage 2 into G.Un (in place).
-// S = explicit sources of the cell, sgE = sqrt(gamma) E^(stage).
+// S = explicit sources of the cell, sgE = sqrt(gamma) E^(stage), un = the cell's U^n, x1 = its calE^(1) (stage 2).
 template <int STAGE>
 __device__ __forceinline__ void stage_precombine(const GridView& G, long long c, double dt, const double S[NCONS],
-                                                 const double sgE[3]) {
+                                                 const double sgE[3], const double un[NCONS], const double x1[3]) {
   const double gam = 1.0 - 0.70710678118654752440;   // 1 - 1/sqrt(2)
   if (STAGE == 1) {
 #pragma unroll
     for (int v = 0; v < NCONS; ++v) {
-      const double un = G.Un[v][c];
-      double u = un + dt * S[v];
+      double u = un[v] + dt * S[v];
       if (v >= CEX && v <= CEZ) {
-        const double R1 = (sgE[v - CEX] - un) / (gam * dt);
+        const double R1 = (sgE[v - CEX] - un[v]) / (gam * dt);
         u += dt * (1.0 - 2.0 * gam) * R1;
       }
       G.Us[v][c] = u;
@@ -168,12 +163,9 @@ __device__ __forceinline__ void stage_precombine(const GridView& G, long long c,
   } else {
 #pragma unroll
     for (int v = 0; v < NCONS; ++v) {
-      const double un = G.Un[v][c], us = G.Us[v][c];
-      double u = 0.5 * (un + us) + 0.5 * dt * S[v];
-      if (v >= CEX && v <= CEZ) {
-        const double x1 = G.X1[v - CEX][c];
-        u += (x1 - un) + (sgE[v - CEX] - us) / (2.0 * gam);
-      }
+      const double us = G.Us[v][c];
+      double u = 0.5 * (un[v] + us) + 0.5 * dt * S[v];
+      if (v >= CEX && v <= CEZ) u += (x1[v - CEX] - un[v]) + (sgE[v - CEX] - us) / (2.0 * gam);
       G.Un[v][c] = u;
     }
   }
