@@ -57,6 +57,26 @@ def load_peaks():
     return 6650.0, "fallback"
 
 
+def roof_kernel(variant: int) -> str:
+    return {0: "k_flux_tma", 1: "k_rhs_simple", 2: "k_rhs_pencil"}[variant]
+
+
+def ncu_traffic(kernel: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
+    (profiles/ncu_traffic.md), or None if that kernel / workload was not captured."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.md")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        c = [x.strip() for x in line.strip().strip("|").split("|")]
+        if len(c) == 3 and c[0] == kernel and c[1] == workload:
+            try:
+                return float(c[2])
+            except ValueError:
+                return None
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons sampled every 100 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -295,8 +315,8 @@ def run_ours(args):
         roof = {"bound": "hbm", "achieved": nbytes_alg / rhs_avg_s / 1e9, "peak": hbm_gbs, "unit": "GB/s",
                 "peak_kind": "%s copy bandwidth (MEASURED_PEAKS.json)" % peak_kind}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
-    roof["kernel"] = {0: "k_flux_tma", 1: "k_rhs_simple", 2: "k_rhs_pencil"}[args.rhs_variant]
+    roof["traffic"] = ncu_traffic(roof_kernel(args.rhs_variant), w.name)
+    roof["kernel"] = roof_kernel(args.rhs_variant)
     roof["avg_launch_ms"] = rhs_avg_s * 1e3
     roof["alg_flops_per_cell"] = RHS_FLOPS[w.recon]
     roof["alg_bytes_per_cell"] = RHS_DOUBLES * 8.0
