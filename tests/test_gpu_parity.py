@@ -263,3 +263,65 @@ def test_api_errors(binding):
     assert L.rgrmhd_step(h, -1.0, 2) == -1
     assert L.rgrmhd_destroy(h) == 0
     assert b"invalid" in L.rgrmhd_strerror(-1)
+
+
+# ----------------------------------------------------------------------------------------------
+# full-size configs, in the launch configuration bench.py times: sampled element-by-element parity
+# ----------------------------------------------------------------------------------------------
+def _sampled_full_size(binding, w, samples, margin=8, nsteps_after=0):
+    """One step of the FULL grid on the GPU; the oracle advances sub-blocks cut out of the same seeded
+    fields (outflow boundaries on the cut faces).  After one step the two agree wherever the numerical
+    domain of dependence (two RHS evaluations x 3 cells, + 2 for the metric derivatives) has not reached a
+    cut face: compare the sub-block minus `margin` cells on every cut side, element by element."""
+    f = w.fields()
+    g = binding.from_workload(w, fields=f)
+    g.step(w.dt, w.recon)
+    Pg = g.get_prims()
+    assert np.isfinite(Pg).all()
+    worst = 0.0
+    for lo, shape in samples:
+        fs = w.fields(lo, shape)
+        o = oracle.from_workload(w, fields=fs, omp=True, n=shape, bc=(wl.BC_OUTFLOW,) * 3)
+        o.step(w.dt, w.recon)
+        Po = interior(o.get_prims(), shape)
+        sl_o, sl_g = [slice(None)], [slice(None)]
+        for d in (2, 1, 0):                                    # arrays are (field, z, y, x)
+            a = 0 if lo[d] == 0 else margin                   # a true domain boundary needs no margin
+            b = shape[d] if lo[d] + shape[d] == w.n[d] else shape[d] - margin
+            sl_o.append(slice(a, b))
+            sl_g.append(slice(3 + lo[d] + a, 3 + lo[d] + b))
+        A, B = Pg[tuple(sl_g)], Po[tuple(sl_o)]
+        err = rel_linf(A, B, prim_group_scales(B, min(w.dx)))
+        assert err.max() <= TOL1, (lo, shape, err)
+        worst = max(worst, err.max())
+    for _ in range(nsteps_after):
+        g.step(w.dt, w.recon)
+    if nsteps_after:
+        assert np.isfinite(g.get_prims()).all()
+    return g, worst
+
+
+def test_cfg4_full_256_sampled(binding):
+    """BASELINE config 4 at its full size (the bench workload): samples across the cylinder edge, in the
+    smooth ambient, and in a domain corner; then the remaining 19 steps stay finite with no failed solve."""
+    w = wl.blast_curved()
+    samples = [((104, 118, 100), (40, 36, 32)), ((20, 200, 60), (36, 32, 32)), ((0, 0, 0), (32, 32, 32)),
+               ((224, 224, 224), (32, 32, 32))]
+    g, _ = _sampled_full_size(binding, w, samples, nsteps_after=19)
+    st = g.stats()
+    assert st["c2p_failures"] == 0 and st["c2p_solves"] == 3 * 20 * 256 ** 3
+
+
+def test_cfg5_full_512_sampled(binding):
+    """BASELINE config 5 at its full size (512^3, ~110 GB of device fields): samples at the centre, across
+    the stellar surface (floor resets active) and in the atmosphere corner."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 125e9:
+        pytest.skip("needs ~110 GB of free device memory")
+    w = wl.tov_like()
+    i_surf = int(round((8.125 + 12.0) / w.dx[0]))
+    samples = [((240, 240, 240), (32, 32, 32)), ((i_surf - 18, 244, 246), (36, 24, 20)), ((0, 0, 0), (28, 28, 28))]
+    g, _ = _sampled_full_size(binding, w, samples)
+    st = g.stats()
+    assert st["floor_resets"] > 0 and st["c2p_solves"] == 3 * 512 ** 3
