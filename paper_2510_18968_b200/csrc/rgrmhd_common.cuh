@@ -298,30 +298,107 @@ __device__ __forceinline__ double weno5_eval(double u0, double u1, double u2, do
   const double a0 = 0.1 * (p12 * p12), a1 = 0.6 * (p02 * p02), a2 = 0.3 * (p01 * p01);
   return (a0 * q0 + a1 * q1 + a2 * q2) * rcp_fast(6.0 * (a0 + a1 + a2));
 }
-// Both face values of the centre cell u2 from one set of smoothness indicators.  Same weights as
-// weno5_eval (d_k / b_k^2 in product form, d = (0.1, 0.6, 0.3) seen from the face), candidates with the
-// 1/6 folded in; lo is the mirror image of hi.
+// Both face values of the centre cell u2 from one set of smoothness indicators.  Same scheme as
+// weno5_eval (Jiang-Shu indicators, weights d_k / (eps + beta_k)^2 with d = (0.1, 0.6, 0.3) seen from the
+// face, in product form: one reciprocal per face value), written in the first differences
+// D_i = u_{i+1} - u_i: the second differences and the candidate values minus u2 are linear in them,
+//   beta_0: d = D1 - D0, e = 3 D1 - D0;  beta_1: d = D2 - D1, e = D1 + D2;  beta_2: d = D3 - D2, e = D3 - 3 D2
+//   q0 - u2 = (5 D1 - 2 D0)/6,  q1 - u2 = (2 D2 + D1)/6,  q2 - u2 = (4 D2 - D3)/6    (upper face; lower = mirror)
+// with the linear weights folded into the candidate coefficients: 64 FP64 instructions for both faces.
 __device__ __forceinline__ void weno5_pair(double u0, double u1, double u2, double u3, double u4, double eps_w,
                                            double& lo, double& hi) {
-  double b0, b1, b2;
-  weno5_beta(u0, u1, u2, u3, u4, eps_w, b0, b1, b2);
+  const double D0 = u1 - u0, D1 = u2 - u1, D2 = u3 - u2, D3 = u4 - u3;
+  const double d0 = D1 - D0, e0 = fma(3.0, D1, -D0);
+  const double d1 = D2 - D1, e1 = D1 + D2;
+  const double d2 = D3 - D2, e2 = fma(-3.0, D2, D3);
+  const double b0 = fma(13.0 / 12.0, d0 * d0, fma(0.25 * e0, e0, eps_w));
+  const double b1 = fma(13.0 / 12.0, d1 * d1, fma(0.25 * e1, e1, eps_w));
+  const double b2 = fma(13.0 / 12.0, d2 * d2, fma(0.25 * e2, e2, eps_w));
   const double p12 = b1 * b2, p02 = b0 * b2, p01 = b0 * b1;
   const double s12 = p12 * p12, s02 = p02 * p02, s01 = p01 * p01;
-  const double wB = 0.6 * s02;
-  const double hA = 0.1 * s12, hC = 0.3 * s01;     // hi: stencils {u0,u1,u2}, {u1,u2,u3}, {u2,u3,u4}
-  const double lA = 0.1 * s01, lC = 0.3 * s12;     // lo: stencils {u4,u3,u2}, {u3,u2,u1}, {u2,u1,u0}
-  constexpr double c13 = 1.0 / 3.0, c76 = 7.0 / 6.0, c116 = 11.0 / 6.0, c16 = 1.0 / 6.0, c56 = 5.0 / 6.0;
-  const double hq0 = fma(c13, u0, fma(-c76, u1, c116 * u2));
-  const double hq1 = fma(-c16, u1, fma(c56, u2, c13 * u3));
-  const double hq2 = fma(c13, u2, fma(c56, u3, -c16 * u4));
-  const double lq0 = fma(c13, u4, fma(-c76, u3, c116 * u2));
-  const double lq1 = fma(-c16, u3, fma(c56, u2, c13 * u1));
-  const double lq2 = fma(c13, u2, fma(c56, u1, -c16 * u0));
-  const double hn = fma(hA, hq0, fma(wB, hq1, hC * hq2)), hd = hA + wB + hC;
-  const double ln = fma(lA, lq0, fma(wB, lq1, lC * lq2)), ld = lA + wB + lC;
-  hi = hn * rcp_fast(hd);
-  lo = ln * rcp_fast(ld);
+  // upper face: stencils {u0,u1,u2}, {u1,u2,u3}, {u2,u3,u4} weighted 0.1 s12, 0.6 s02, 0.3 s01
+  const double hA = fma(0.1 * 5.0 / 6.0, D1, (-0.1 * 2.0 / 6.0) * D0);
+  const double hB = fma(0.6 * 2.0 / 6.0, D2, (0.6 / 6.0) * D1);
+  const double hC = fma(0.3 * 4.0 / 6.0, D2, (-0.3 / 6.0) * D3);
+  const double hn = fma(s12, hA, fma(s02, hB, s01 * hC));
+  const double hd = fma(0.1, s12, fma(0.6, s02, 0.3 * s01));
+  // lower face: the mirror image (u0 <-> u4, u1 <-> u3: D_i -> -D_{3-i}, beta_0 <-> beta_2)
+  const double lA = fma(-0.1 * 5.0 / 6.0, D2, (0.1 * 2.0 / 6.0) * D3);
+  const double lB = fma(-0.6 * 2.0 / 6.0, D1, (-0.6 / 6.0) * D2);
+  const double lC = fma(-0.3 * 4.0 / 6.0, D1, (0.3 / 6.0) * D0);
+  const double ln = fma(s01, lA, fma(s02, lB, s12 * lC));
+  const double ld = fma(0.1, s01, fma(0.6, s02, 0.3 * s12));
+  hi = fma(hn, rcp_fast(hd), u2);
+  lo = fma(ln, rcp_fast(ld), u2);
 }
+// N independent cells at once, statement by statement across the cells, so that the instruction stream
+// interleaves N dependency chains (the reciprocal tails are serial: seed + 4 dependent DFMA).
+template <int N>
+__device__ __forceinline__ void weno5_pair_n(const double (&u)[N][5], double eps_w, double (&lo)[N], double (&hi)[N]) {
+  double D0[N], D1[N], D2[N], D3[N], b0[N], b1[N], b2[N], s12[N], s02[N], s01[N], hn[N], hd[N], ln[N], ld[N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) { D0[j] = u[j][1] - u[j][0]; D1[j] = u[j][2] - u[j][1]; D2[j] = u[j][3] - u[j][2]; D3[j] = u[j][4] - u[j][3]; }
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double d0 = D1[j] - D0[j], e0 = fma(3.0, D1[j], -D0[j]);
+    const double d1 = D2[j] - D1[j], e1 = D1[j] + D2[j];
+    const double d2 = D3[j] - D2[j], e2 = fma(-3.0, D2[j], D3[j]);
+    b0[j] = fma(13.0 / 12.0, d0 * d0, fma(0.25 * e0, e0, eps_w));
+    b1[j] = fma(13.0 / 12.0, d1 * d1, fma(0.25 * e1, e1, eps_w));
+    b2[j] = fma(13.0 / 12.0, d2 * d2, fma(0.25 * e2, e2, eps_w));
+  }
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double p12 = b1[j] * b2[j], p02 = b0[j] * b2[j], p01 = b0[j] * b1[j];
+    s12[j] = p12 * p12; s02[j] = p02 * p02; s01[j] = p01 * p01;
+  }
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double hA = fma(0.1 * 5.0 / 6.0, D1[j], (-0.1 * 2.0 / 6.0) * D0[j]);
+    const double hB = fma(0.6 * 2.0 / 6.0, D2[j], (0.6 / 6.0) * D1[j]);
+    const double hC = fma(0.3 * 4.0 / 6.0, D2[j], (-0.3 / 6.0) * D3[j]);
+    hn[j] = fma(s12[j], hA, fma(s02[j], hB, s01[j] * hC));
+    hd[j] = fma(0.1, s12[j], fma(0.6, s02[j], 0.3 * s01[j]));
+    const double lA = fma(-0.1 * 5.0 / 6.0, D2[j], (0.1 * 2.0 / 6.0) * D3[j]);
+    const double lB = fma(-0.6 * 2.0 / 6.0, D1[j], (-0.6 / 6.0) * D2[j]);
+    const double lC = fma(-0.3 * 4.0 / 6.0, D1[j], (0.3 / 6.0) * D0[j]);
+    ln[j] = fma(s01[j], lA, fma(s02[j], lB, s12[j] * lC));
+    ld[j] = fma(0.1, s01[j], fma(0.6, s02[j], 0.3 * s12[j]));
+  }
+  // 2N reciprocals, Newton steps interleaved
+  double r[2 * N], e[2 * N], x[2 * N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) { x[2 * j] = hd[j]; x[2 * j + 1] = ld[j]; }
+#pragma unroll
+  for (int q = 0; q < 2 * N; ++q) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r[q]) : "d"(x[q]));
+#pragma unroll
+  for (int q = 0; q < 2 * N; ++q) e[q] = fma(-x[q], r[q], 1.0);
+#pragma unroll
+  for (int q = 0; q < 2 * N; ++q) r[q] = fma(r[q], e[q], r[q]);
+#pragma unroll
+  for (int q = 0; q < 2 * N; ++q) e[q] = fma(-x[q], r[q], 1.0);
+#pragma unroll
+  for (int q = 0; q < 2 * N; ++q) r[q] = fma(r[q], e[q], r[q]);
+#pragma unroll
+  for (int j = 0; j < N; ++j) { hi[j] = fma(hn[j], r[2 * j], u[j][2]); lo[j] = fma(ln[j], r[2 * j + 1], u[j][2]); }
+}
+
+// reconstruction of N cells at once (lo/hi = values at each cell's lower/upper face)
+template <int RECON, int N>
+__device__ __forceinline__ void recon_cells(double eps_w, const double (&u)[N][5], double (&lo)[N], double (&hi)[N]) {
+  if (RECON == RECON_WENO5) {
+    weno5_pair_n<N>(u, eps_w, lo, hi);
+  } else {
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+      const double a = u[j][2] - u[j][1], b = u[j][3] - u[j][2];
+      const double slope = (RECON == RECON_MINMOD) ? minmod2(a, b) : minmod3(2.0 * a, 2.0 * b, 0.5 * (a + b));
+      hi[j] = u[j][2] + 0.5 * slope;
+      lo[j] = u[j][2] - 0.5 * slope;
+    }
+  }
+}
+
 template <int RECON>
 __device__ __forceinline__ void recon_cell(double eps_w, double um2, double um1, double u0, double up1, double up2,
                                            double& lo, double& hi) {

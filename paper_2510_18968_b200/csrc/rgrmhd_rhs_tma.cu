@@ -259,12 +259,20 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           if (howner) lds_stencil<RECON>(&S.ring[s1][hal0], sst, u[1]);
         }
         if (howner) {                                                  // halo cells of this pair (x, y only)
+          double l2[2], h2[2];
+          if (two) {
+            recon_cells<RECON, 2>(G.weno_eps, u, l2, h2);
+          } else {
+            double l1[1], h1[1];
+            const double (&c1)[1][5] = reinterpret_cast<const double (&)[1][5]>(u);
+            recon_cells<RECON, 1>(G.weno_eps, c1, l1, h1);
+            l2[0] = l1[0]; h2[0] = h1[0];
+          }
 #pragma unroll
           for (int j = 0; j < 2; ++j) {
             if (j == 0 || two) {
               const int vr = v0 + j;
-              double l, h;
-              recon_cell<RECON>(G.weno_eps, u[j][0], u[j][1], u[j][2], u[j][3], u[j][4], l, h);
+              double l = l2[j], h = h2[j];
               if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
                 if (!(l > 0.0)) l = u[j][2];
                 if (!(h > 0.0)) h = u[j][2];
@@ -302,19 +310,29 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           if (v + 4 < NV) probe(v + 4);
         }
         if (v == VRAW && solve) load_face_raw(T, K, cl, cr, raw);     // consumed after the loop
+        {
+          double l2[2], h2[2];
+          if (v + 1 < NV) {
+            recon_cells<RECON, 2>(G.weno_eps, cur, l2, h2);
+          } else {
+            double l1[1], h1[1];
+            const double (&c1)[1][5] = reinterpret_cast<const double (&)[1][5]>(cur);
+            recon_cells<RECON, 1>(G.weno_eps, c1, l1, h1);
+            l2[0] = l1[0]; h2[0] = h1[0];
+          }
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-          if (v + j < NV) {
-            const int vr = v + j;
-            double l, h;
-            recon_cell<RECON>(G.weno_eps, cur[j][0], cur[j][1], cur[j][2], cur[j][3], cur[j][4], l, h);
-            if (vr < 2) {
-              if (!(l > 0.0)) l = cur[j][2];
-              if (!(h > 0.0)) h = cur[j][2];
+          for (int j = 0; j < 2; ++j) {
+            if (v + j < NV) {
+              const int vr = v + j;
+              double l = l2[j], h = h2[j];
+              if (vr < 2) {
+                if (!(l > 0.0)) l = cur[j][2];
+                if (!(h > 0.0)) h = cur[j][2];
+              }
+              lo[vr] = l;
+              hi_dst[vr * hi_str] = h;
+              if (edge) S.exhi[vr][(K == 0) ? ty : tx] = h;
             }
-            lo[vr] = l;
-            hi_dst[vr * hi_str] = h;
-            if (edge) S.exhi[vr][(K == 0) ? ty : tx] = h;
           }
         }
 #pragma unroll
