@@ -69,10 +69,9 @@ __device__ __forceinline__ void implicit_E_closed(const double v[3], double W, d
 }
 
 // P holds the guess (rho, p, v^i) on entry and all 14 primitives on return.  sg = sqrt(gamma).
-__device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double alpha, double Gamma,
+__device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double alpha, double Gamma,
                                             const double U[NCONS], double adt, double sigma, double tol, int maxit,
                                             double P[NPRIM]) {
-  const double isg = rcp_fast(sg);
   const double gm1og = (Gamma - 1.0) / Gamma;
   const double Dh = U[CD] * isg, tauh = U[CTAU] * isg;
   double Sh[3], Es[3], B[3], EsxB[3];
@@ -87,6 +86,7 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double al
   cross3(Es, B, EsxB);
   const double s0 = adt * alpha * sigma;
   const double escale = sqrt(dot3(Es, Es) + B2);
+  const double ies = escale > 0.0 ? 1.0 / escale : 1.0;
   C2POut res = {0, 1};
   const double Zlo = Dh, Zhi = Gamma * (tauh + Dh - 0.5 * B2);
   // guess
@@ -128,7 +128,7 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double al
         double N[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) N[i] = Sh[i] - EsxB[i] * i1s;
-        const double fpar = (B2 > 0.0) ? dot3(N, B) / B2 : 0.0;
+        const double fpar = (B2 > 1e-280) ? dot3(N, B) * rcp_fast(B2) : (B2 > 0.0) ? dot3(N, B) / B2 : 0.0;
 #pragma unroll
         for (int i = 0; i < 3; ++i) { Npar[i] = fpar * B[i]; Nperp[i] = N[i] - Npar[i]; }
         cross3(B, Nperp, BxN);
@@ -191,13 +191,12 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double sg, double al
             converged = true; done = true;
           } else {
             // Anderson(1) acceleration of x -> G(x), x = (W, kE/escale)
-            const double es = escale > 0.0 ? escale : 1.0;
-            const double fW = Wnew - W, fk = (kEnew - kE) / es;
+            const double fW = Wnew - W, fk = (kEnew - kE) * ies;
             double Wnext = Wnew, knext = kEnew;
             if (outer > 0) {
               const double dW = fW - fW_prev, dk = fk - fk_prev, den = dW * dW + dk * dk;
               if (den > 0.0) {
-                const double theta = (fW * dW + fk * dk) / den;
+                const double theta = (fW * dW + fk * dk) * rcp_fast(den);
                 const double Wa = Wnew - theta * (Wnew - GW_prev), ka = kEnew - theta * (kEnew - Gk_prev);
                 if (isfinite(Wa) && isfinite(ka) && Wa >= 1.0 && fabs(theta) < 10.0) { Wnext = Wa; knext = ka; }
               }
@@ -271,7 +270,8 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
     for (int v = 0; v < NCONS; ++v) U[v] = Ust[v][c];
 #pragma unroll
     for (int v = 0; v < 5; ++v) P[v] = G.P[v][c];
-    const double sigma = (STAGE == 3) ? 0.0 : sigma_of(G, U[CD] / sg, c);
+    const double isg = rcp_fast(sg);
+    const double sigma = (STAGE == 3) ? 0.0 : sigma_of(G, U[CD] * isg, c);
     // The point-wise right-hand side after the solve reads ~57 more fields of this cell.  Start those loads
     // now as asynchronous copies into a thread-private shared-memory column: no registers are held and
     // the solve below hides their DRAM latency.
@@ -291,7 +291,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
-    C2POut r2 = c2p_solve(t, sg, alpha, G.Gamma, U, adt, sigma, G.tol, G.maxit, P);
+    C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, U, adt, sigma, G.tol, G.maxit, P);
     evals = r2.evals; failed = r2.failed;
     if (G.rho_floor > 0.0 && (r2.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
       // reading R9: atmosphere reset
@@ -300,7 +300,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       P[PRS] = G.p_atmo;
       const double s = adt * alpha * sigma;
 #pragma unroll
-      for (int q = 0; q < 3; ++q) P[EX + q] = (U[CEX + q] / sg) / (1.0 + s);
+      for (int q = 0; q < 3; ++q) P[EX + q] = (U[CEX + q] * isg) / (1.0 + s);
       if (STAGE == 3) {
         Met m;
         load_met_cell(G, c, m);
@@ -314,11 +314,12 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
 #pragma unroll
     for (int v = 0; v < NPRIM; ++v) G.P[v][c] = P[v];
     double sgE[3];
+    const double iada = (STAGE == 3) ? 0.0 : rcp_fast(adt * alpha);
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
       sgE[q] = sg * P[EX + q];
       if (STAGE == 1) G.X1[q][c] = sgE[q];
-      G.jc[q][c] = (STAGE == 3) ? 0.0 : (U[CEX + q] / sg - P[EX + q]) / (adt * alpha);
+      G.jc[q][c] = (STAGE == 3) ? 0.0 : (U[CEX + q] * isg - P[EX + q]) * iada;
     }
     if (STAGE != 3) {
       // ---- a4 + a5 (point-wise part)

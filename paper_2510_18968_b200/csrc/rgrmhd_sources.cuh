@@ -150,14 +150,12 @@ template <int STAGE>
 __device__ __forceinline__ void stage_precombine(const GridView& G, long long c, double dt, const double S[NCONS],
                                                  const double sgE[3], const double un[NCONS], const double x1[3]) {
   const double gam = 1.0 - 0.70710678118654752440;   // 1 - 1/sqrt(2)
+  const double c1 = (1.0 - 2.0 * gam) / gam, c2 = 1.0 / (2.0 * gam);   // compile-time constants
   if (STAGE == 1) {
 #pragma unroll
     for (int v = 0; v < NCONS; ++v) {
       double u = un[v] + dt * S[v];
-      if (v >= CEX && v <= CEZ) {
-        const double R1 = (sgE[v - CEX] - un[v]) / (gam * dt);
-        u += dt * (1.0 - 2.0 * gam) * R1;
-      }
+      if (v >= CEX && v <= CEZ) u += c1 * (sgE[v - CEX] - un[v]);       // dt (1 - 2 gamma) R1, R1 = (X1 - X^n)/(gamma dt)
       G.Us[v][c] = u;
     }
   } else {
@@ -165,7 +163,7 @@ __device__ __forceinline__ void stage_precombine(const GridView& G, long long c,
     for (int v = 0; v < NCONS; ++v) {
       const double us = G.Us[v][c];
       double u = 0.5 * (un[v] + us) + 0.5 * dt * S[v];
-      if (v >= CEX && v <= CEZ) u += (x1[v - CEX] - un[v]) + (sgE[v - CEX] - us) / (2.0 * gam);
+      if (v >= CEX && v <= CEZ) u += (x1[v - CEX] - un[v]) + c2 * (sgE[v - CEX] - us);
       G.Un[v][c] = u;
     }
   }
