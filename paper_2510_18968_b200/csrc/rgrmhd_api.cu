@@ -135,6 +135,8 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   }
   G.stride[0] = 1; G.stride[1] = G.np[0]; G.stride[2] = (long long)G.np[0] * G.np[1];
   G.Gamma = p->gamma_eos;
+  G.gog1 = p->gamma_eos / (p->gamma_eos - 1.0);
+  G.gm1og = (p->gamma_eos - 1.0) / p->gamma_eos;
   G.sigma_model = p->sigma_model; G.sigma0 = p->sigma0; G.sigma_dref = p->sigma_dref;
   G.sigma_exp = (int)std::lround(p->sigma_exp);
   G.kappa = p->kappa;

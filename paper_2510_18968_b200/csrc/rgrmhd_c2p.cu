@@ -69,10 +69,9 @@ __device__ __forceinline__ void implicit_E_closed(const double v[3], double W, d
 }
 
 // P holds the guess (rho, p, v^i) on entry and all 14 primitives on return.  sg = sqrt(gamma).
-__device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double alpha, double Gamma,
-                                            const double U[NCONS], double adt, double sigma, double tol, int maxit,
-                                            double P[NPRIM]) {
-  const double gm1og = (Gamma - 1.0) / Gamma;
+__device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double alpha, double Gamma, double gog1,
+                                            double gm1og, const double U[NCONS], double adt, double sigma, double tol,
+                                            int maxit, double P[NPRIM]) {
   const double Dh = U[CD] * isg, tauh = U[CTAU] * isg;
   double Sh[3], Es[3], B[3], EsxB[3];
   triad_from_cov(t, U[CSX] * isg, U[CSY] * isg, U[CSZ] * isg, Sh);
@@ -85,8 +84,10 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
   const double B2 = dot3(B, B);
   cross3(Es, B, EsxB);
   const double s0 = adt * alpha * sigma;
-  const double escale = sqrt(dot3(Es, Es) + B2);
-  const double ies = escale > 0.0 ? 1.0 / escale : 1.0;
+  const double em2 = dot3(Es, Es) + B2;
+  double escale, ies;
+  if (em2 > 1e-280) sqrt_rsqrt_fast(em2, escale, ies);
+  else { escale = sqrt(em2); ies = escale > 0.0 ? 1.0 / escale : 1.0; }
   C2POut res = {0, 1};
   const double Zlo = Dh, Zhi = Gamma * (tauh + Dh - 0.5 * B2);
   // guess
@@ -104,12 +105,12 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
     P[EX] = EU[0]; P[EY] = EU[1]; P[EZ] = EU[2];
     return res;
   }
-  double Z = (P[RHO] + Gamma / (Gamma - 1.0) * P[PRS]) * W * W;
+  double Z = (P[RHO] + gog1 * P[PRS]) * W * W;
   bool converged = false, state_ok = false;
   const int max_outer = 50;
   // inverse slope of g for the first secant step: dg/dZ ~ 1 - (Gamma-1)/Gamma / W^2 at fixed v (exact in the
   // unmagnetised, slow limit), instead of 1
-  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, islope = 1.0 / (1.0 - gm1og * (1.0 - v2g));
+  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, islope = rcp_fast(1.0 - gm1og * (1.0 - v2g));
   // frozen per outer pass
   double s = 0, r = 0, i1s = 1, Npar[3] = {0, 0, 0}, Nperp[3] = {0, 0, 0}, BxN[3] = {0, 0, 0};
   // last evaluation
@@ -291,7 +292,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
-    C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, U, adt, sigma, G.tol, G.maxit, P);
+    C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, P);
     evals = r2.evals; failed = r2.failed;
     if (G.rho_floor > 0.0 && (r2.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
       // reading R9: atmosphere reset

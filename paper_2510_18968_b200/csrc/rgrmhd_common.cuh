@@ -36,6 +36,7 @@ struct GridView {
   long long ntot;
   double dx[3], inv_dx[3], inv_12dx[3];
   double Gamma, sigma0, sigma_dref, kappa, rho_floor, p_atmo, tol, weno_eps;
+  double gog1, gm1og;    // Gamma/(Gamma-1), (Gamma-1)/Gamma (host-computed: no division in the kernels)
   int sigma_model, sigma_exp, maxit, charge_mode;
   const double* met[NMET];
   const double* sigma;   // SIGMA_ARRAY only, else nullptr

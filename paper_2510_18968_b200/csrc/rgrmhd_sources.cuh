@@ -82,7 +82,7 @@ __device__ __forceinline__ void add_sources(const GridView& G, const Met& m, con
   lower(m, vU, vD); lower(m, EU, ED); lower(m, BU, BD);
   cross_raw(EU, BU, ExB);
   const double v2 = dot3(vU, vD), W2 = rcp_fast(1.0 - v2);
-  const double h = rho + G.Gamma / (G.Gamma - 1.0) * p;
+  const double h = rho + G.gog1 * p;
   const double pem = 0.5 * (dot3(EU, ED) + dot3(BU, BD)), hW2 = h * W2;
   const double al = m.alpha, sg = m.sg;
   // T^ab = h W^2 v^a v^b + g^ab (p + (E^2+B^2)/2) - E^a E^b - B^a B^b, stored with the symmetric-contraction
