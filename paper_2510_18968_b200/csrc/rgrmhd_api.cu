@@ -152,11 +152,12 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   const size_t bytes = (size_t)nfields * (size_t)h->field_stride * sizeof(double);
   cudaError_t e = cudaMalloc((void**)&h->slab, bytes);
   if (e != cudaSuccess) { cudaGetLastError(); delete h; return RGRMHD_E_NOMEM; }
-  e = cudaMalloc((void**)&h->stats_dev, sizeof(rg::StatsDev) + sizeof(unsigned long long));
+  e = cudaMalloc((void**)&h->stats_dev, sizeof(rg::StatsDev) + 2 * sizeof(unsigned long long));
   if (e != cudaSuccess) { cudaGetLastError(); cudaFree(h->slab); delete h; return RGRMHD_E_NOMEM; }
   h->maxspeed_dev = (unsigned long long*)(h->stats_dev + 1);
   cudaMemset(h->slab, 0, bytes);
-  cudaMemset(h->stats_dev, 0, sizeof(rg::StatsDev) + sizeof(unsigned long long));
+  cudaMemset(h->stats_dev, 0, sizeof(rg::StatsDev) + 2 * sizeof(unsigned long long));
+  G.src_mask = h->maxspeed_dev + 1;
   double* q = h->slab;
   auto next = [&]() { double* r = q; q += h->field_stride; return r; };
   for (int v = 0; v < rg::NMET; ++v) G.met[v] = next();

@@ -238,7 +238,8 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
 // The guess is the current G.P.  jc = undensitised conduction current of the stage (reading R3).
 constexpr int C2P_TX = 32, C2P_TY = 4;
 // staging slots of the point-wise right-hand side (doubles per thread)
-enum { PF_SRC = 0, PF_K = NSRC, PF_UN = NSRC + 6, PF_X1 = NSRC + 6 + NCONS, PF_COUNT = NSRC + 6 + NCONS + 3 };
+enum { PF_SRC = 0, PF_K = NSRC, PF_UN = NSRC + 6, PF_X1 = NSRC + 6 + NCONS, PF_US = NSRC + 6 + NCONS + 3,
+       PF_COUNT1 = PF_X1, PF_COUNT2 = PF_US + NCONS };
 __device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src)
                : "memory");
@@ -280,15 +281,25 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
     double* const pf = pf_smem + threadIdx.x;              // pf[q * NTH]: conflict-free, private to this thread
     constexpr int NTH = C2P_TX * C2P_TY;
     if (STAGE != 3) {
+      // fields that are identically zero on this grid (zero shift, K_ij = 0, diagonal metric, ...) are not read
+      const unsigned long long nz = __ldg(G.src_mask);
 #pragma unroll
-      for (int q = 0; q < NSRC; ++q) cp_async8(pf + (PF_SRC + q) * NTH, G.src[q] + c);
+      for (int q = 0; q < NSRC; ++q) {
+        if ((nz >> q) & 1ull) cp_async8(pf + (PF_SRC + q) * NTH, G.src[q] + c);
+        else pf[(PF_SRC + q) * NTH] = 0.0;
+      }
 #pragma unroll
-      for (int q = 0; q < 6; ++q) cp_async8(pf + (PF_K + q) * NTH, G.met[MKXX + q] + c);
+      for (int q = 0; q < 6; ++q) {
+        if ((nz >> (NSRC + q)) & 1ull) cp_async8(pf + (PF_K + q) * NTH, G.met[MKXX + q] + c);
+        else pf[(PF_K + q) * NTH] = 0.0;
+      }
 #pragma unroll
       for (int v = 0; v < NCONS; ++v) cp_async8(pf + (PF_UN + v) * NTH, G.Un[v] + c);
       if (STAGE == 2) {
 #pragma unroll
         for (int q = 0; q < 3; ++q) cp_async8(pf + (PF_X1 + q) * NTH, G.X1[q] + c);
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) cp_async8(pf + (PF_US + v) * NTH, G.Us[v] + c);
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
@@ -330,7 +341,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       Met m;
       load_met_cell(G, c, m);
       asm volatile("cp.async.wait_group 0;" ::: "memory");
-      double src[NSRC], Kq[6], un[NCONS], x1[3] = {0.0, 0.0, 0.0};
+      double src[NSRC], Kq[6], un[NCONS], us[NCONS], x1[3] = {0.0, 0.0, 0.0};
 #pragma unroll
       for (int q = 0; q < NSRC; ++q) src[q] = pf[(PF_SRC + q) * NTH];
 #pragma unroll
@@ -341,8 +352,10 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       if (STAGE == 2) {
 #pragma unroll
         for (int q = 0; q < 3; ++q) x1[q] = pf[(PF_X1 + q) * NTH];
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) us[v] = pf[(PF_US + v) * NTH];
       }
-      stage_precombine<STAGE>(G, c, dt, S, sgE, un, x1);
+      stage_precombine<STAGE>(G, c, dt, S, sgE, un, us, x1);
     }
   }
   // stats: warp reduce, one atomic per warp
@@ -380,23 +393,39 @@ k_prim2cons(const __grid_constant__ GridView G) {
 
 // Static source coefficients of every interior cell (once per set_metric).
 __global__ void __launch_bounds__(128)
-k_metric_coeffs(const __grid_constant__ GridView G) {
+k_metric_coeffs(const __grid_constant__ GridView G, unsigned long long* __restrict__ mask) {
   const int nx = G.n[0], ny = G.n[1];
   const long long nint = (long long)nx * ny * G.n[2];
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nint) return;
-  const int i = (int)(t % nx);
-  const long long r = t / nx;
-  const long long c = cell_index(G, i, (int)(r % ny), (int)(r / ny));
-  double out[NSRC];
-  metric_coeffs_cell(G, c, out);
+  unsigned long long nz = 0;
+  if (t < nint) {
+    const int i = (int)(t % nx);
+    const long long r = t / nx;
+    const long long c = cell_index(G, i, (int)(r % ny), (int)(r / ny));
+    double out[NSRC];
+    metric_coeffs_cell(G, c, out);
 #pragma unroll
-  for (int q = 0; q < NSRC; ++q) G.src[q][c] = out[q];
+    for (int q = 0; q < NSRC; ++q) {
+      G.src[q][c] = out[q];
+      if (out[q] != 0.0) nz |= 1ull << q;
+    }
+#pragma unroll
+    for (int q = 0; q < 6; ++q)
+      if (__ldg(G.met[MKXX + q] + c) != 0.0) nz |= 1ull << (NSRC + q);
+  }
+  // which fields are not identically zero: warp OR, one atomic per warp
+  unsigned lo = (unsigned)nz, hi = (unsigned)(nz >> 32);
+  lo = __reduce_or_sync(0xffffffffu, lo);
+  hi = __reduce_or_sync(0xffffffffu, hi);
+  if ((threadIdx.x & 31) == 0 && (lo | hi)) atomicOr(mask, ((unsigned long long)hi << 32) | lo);
 }
 
 cudaError_t launch_metric_coeffs(const GridView& G, cudaStream_t st) {
   const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
-  k_metric_coeffs<<<(unsigned)((nint + 127) / 128), 128, 0, st>>>(G);
+  unsigned long long* mask = const_cast<unsigned long long*>(G.src_mask);
+  cudaError_t e = cudaMemsetAsync(mask, 0, sizeof(unsigned long long), st);
+  if (e != cudaSuccess) return e;
+  k_metric_coeffs<<<(unsigned)((nint + 127) / 128), 128, 0, st>>>(G, mask);
   return cudaGetLastError();
 }
 
@@ -405,12 +434,13 @@ cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats,
   const dim3 block(C2P_TX * C2P_TY, 1, 1);
   const dim3 grid((G.n[0] + C2P_TX - 1) / C2P_TX, (G.n[1] + C2P_TY - 1) / C2P_TY, G.n[2]);
   if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
-  const size_t smem = (size_t)PF_COUNT * C2P_TX * C2P_TY * sizeof(double);
+  size_t smem = (size_t)PF_COUNT1 * C2P_TX * C2P_TY * sizeof(double);
   cudaError_t e;
   if (stage == 1) {
     if ((e = cudaFuncSetAttribute(k_c2p<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
     k_c2p<1><<<grid, block, smem, st>>>(G, dt, stats);
   } else if (stage == 2) {
+    smem = (size_t)PF_COUNT2 * C2P_TX * C2P_TY * sizeof(double);
     if ((e = cudaFuncSetAttribute(k_c2p<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
     k_c2p<2><<<grid, block, smem, st>>>(G, dt, stats);
   } else {

@@ -46,6 +46,7 @@ struct GridView {
   double* Us[NCONS];     // stage vector U*^(2)
   double* X1[3];         // calE^(1) (needed again by the final combine, Eq. 37)
   double* src[NSRC];     // static source coefficients (metric derivatives, G^i, tr K; rgrmhd_sources.cuh)
+  const unsigned long long* src_mask;   // device word: bit q set <=> src[q] (q < NSRC) / K_ij[q - NSRC] is not identically 0
 };
 
 struct StatsDev {

@@ -145,10 +145,11 @@ __device__ __forceinline__ void add_sources(const GridView& G, const Met& m, con
 //   STAGE 1:  U*2     = [U^n + dt S1 + (1-2 gamma)/gamma (X1 - X^n)|_X]                        - dt div F1
 //   STAGE 2:  U^{n+1} = [(U^n + U*2)/2 + dt/2 S2 + ((X1 - X^n) + (X2 - X*2)/(2 gamma))|_X]   - dt/2 div F2
 // (dt F1 is carried by U*2).  This function writes the bracket: stage 1 into G.Us, stage 2 into G.Un (in place).
-// S = explicit sources of the cell, sgE = sqrt(gamma) E^(stage), un = the cell's U^n, x1 = its calE^(1) (stage 2).
+// S = explicit sources of the cell, sgE = sqrt(gamma) E^(stage), un / us = the cell's U^n / U*2 (us: stage 2), x1 = its calE^(1) (stage 2).
 template <int STAGE>
 __device__ __forceinline__ void stage_precombine(const GridView& G, long long c, double dt, const double S[NCONS],
-                                                 const double sgE[3], const double un[NCONS], const double x1[3]) {
+                                                 const double sgE[3], const double un[NCONS], const double us[NCONS],
+                                                 const double x1[3]) {
   const double gam = 1.0 - 0.70710678118654752440;   // 1 - 1/sqrt(2)
   const double c1 = (1.0 - 2.0 * gam) / gam, c2 = 1.0 / (2.0 * gam);   // compile-time constants
   if (STAGE == 1) {
@@ -161,9 +162,8 @@ __device__ __forceinline__ void stage_precombine(const GridView& G, long long c,
   } else {
 #pragma unroll
     for (int v = 0; v < NCONS; ++v) {
-      const double us = G.Us[v][c];
-      double u = 0.5 * (un[v] + us) + 0.5 * dt * S[v];
-      if (v >= CEX && v <= CEZ) u += (x1[v - CEX] - un[v]) + c2 * (sgE[v - CEX] - us);
+      double u = 0.5 * (un[v] + us[v]) + 0.5 * dt * S[v];
+      if (v >= CEX && v <= CEZ) u += (x1[v - CEX] - un[v]) + c2 * (sgE[v - CEX] - us[v]);
       G.Un[v][c] = u;
     }
   }
