@@ -19,7 +19,7 @@
 // run-time cyclic rotation of the vector/tensor components (cyclic permutations keep the Levi-Civita
 // sign, so Eq. 27 is form invariant), realised for free as index arithmetic on pointer tables and
 // shared-memory planes.  This keeps the kernel ~4x smaller than the fully templated version, whose
-// instruction-cache misses dominated its stall profile (profiles/r01_rhs_tiled_ncu.md).
+// instruction-cache misses dominated its stall profile.
 // Stencils are read straight from global memory (x: coalesced rows, L1; y: L1; z: L2).
 #include "rgrmhd_flux_rot.cuh"
 
