@@ -397,3 +397,30 @@ def test_degenerate_physics(binding, case):
         if case == "hydro":
             Pg = g.get_prims()
             assert not Pg[wl.EX:wl.QCH + 1].any()                       # the EM sector stays identically zero
+
+
+# ----------------------------------------------------------------------------------------------
+# physics at full size, against what the paper fixes (not against the oracle)
+# ----------------------------------------------------------------------------------------------
+def test_cfg3_full_128_exact_alfven_wave_and_conservation(binding):
+    """BASELINE config 3 at its full size: after 20 steps B is the initial circularly polarised Alfven wave
+    (Eq. 56-59) shifted by v_A t along (1,1,1)/sqrt(3) to truncation error (pin <= 1e-4 B0),
+    v to the O(dt) offset of reading R12; total D and total charge are conserved to round-off (zero sources,
+    PAPER.md:153; flat space: also tau, S_i, B^i)."""
+    w = wl.alfven3d()
+    g = binding.from_workload(w)
+    n = w.n
+    U0 = interior(g.get_cons(), n).sum(axis=(1, 2, 3))
+    A0 = np.abs(interior(g.get_cons(), n)).sum(axis=(1, 2, 3))
+    for _ in range(w.nsteps):
+        g.step(w.dt, w.recon)
+    P = g.get_prims()
+    (X, Y, Z), _ = w.coords()
+    B, v, E = wl.alfven_exact(w, X, Y, Z, w.nsteps * w.dt)
+    eB = max(np.max(np.abs(interior(P[wl.BX + i] - B[i], n))) for i in range(3))
+    ev = max(np.max(np.abs(interior(P[wl.VX + i] - v[i], n))) for i in range(3))
+    assert eB <= 1e-4 and ev <= 1e-2, (eB, ev)
+    assert g.stats()["c2p_failures"] == 0
+    U1 = interior(g.get_cons(), n).sum(axis=(1, 2, 3))
+    for i in (0, 1, 2, 3, 4, 8, 9, 10, 13):
+        assert abs(U1[i] - U0[i]) <= 1e-12 * max(A0[i], A0[0] * 1e-3), (i, U0[i], U1[i])
