@@ -286,12 +286,6 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
             }
           }
         }
-        // make sure every lane's stencil values have landed in registers before the stage is released
-        {
-          double sink = dst[0][0] + dst[0][1] + dst[0][2] + dst[0][3] + dst[0][4];
-          if (two) sink += dst[1][0] + dst[1][1] + dst[1][2] + dst[1][3] + dst[1][4];
-          asm volatile("" ::"d"(sink) : "memory");
-        }
         // The stencils were read through the generic proxy; the refill of this stage is an async-proxy (TMA)
         // write.  Without this cross-proxy fence the refill can overtake the reads: measured on B200 as run-to-run
         // differences in ~0.1 % of the cells (always the last box of a z phase, whose stage is refilled at once).
