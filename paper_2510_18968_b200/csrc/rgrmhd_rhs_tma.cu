@@ -32,6 +32,10 @@ constexpr int NWC = NT / 32;                       // compute warps
 constexpr int NTHREADS = NT + 64;                  // + producer warp + edge-face warp
 constexpr int EXW = TX + 1, EXH = TY + 1, EXP = EXW * EXH;
 constexpr int NS = 5;                              // ring stages
+#ifndef RG_GROUP
+#define RG_GROUP 2
+#endif
+constexpr int GR = RG_GROUP;                       // variables reconstructed per step (interleaved dependency chains)
 // The TMA engine needs a 16-byte aligned box origin (an even x coordinate for doubles: an odd one traps with
 // "illegal instruction"), and the ghost offset is 3: the y and z boxes therefore start one cell left of the tile
 // and are TX + 2 wide.
@@ -240,50 +244,52 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
       double* const hi_dst = (K == 2) ? &S.chi[(k & 1)][0][tid] : &S.ex[0][base + up];
       const int hi_str = (K == 2) ? NT : EXP;
       FaceRaw raw;
-      double lo[NVR], cur[2][5], nxt[2][5];
-      unsigned rdy0 = 0, rdy1 = 0;                                     // probe results for the next pair's boxes
-      auto fetch = [&](int v0, double (&dst)[2][5], unsigned r0, unsigned r1) {
-        const int s0 = st;
-        const unsigned p0 = ph;
-        const int s1 = (s0 + 1 == NS) ? 0 : s0 + 1;
-        const unsigned p1 = (s0 + 1 == NS) ? p0 ^ 1u : p0;
-        const bool two = v0 + 1 < NV;
-        const bool howner = K < 2 && warp == (v0 >> 1) % NWC;
-        double u[2][5];
-        if (!r0) mbar_wait(&S.full[s0], p0);
-        asm volatile("" ::: "memory");                                 // no shared-memory load may move above the test of r0
-        lds_stencil<RECON>(&S.ring[s0][own0], sst, dst[0]);
-        if (howner) lds_stencil<RECON>(&S.ring[s0][hal0], sst, u[0]);
-        if (two) {
-          if (!r1) mbar_wait(&S.full[s1], p1);
-          asm volatile("" ::: "memory");
-          lds_stencil<RECON>(&S.ring[s1][own0], sst, dst[1]);
-          if (howner) lds_stencil<RECON>(&S.ring[s1][hal0], sst, u[1]);
-        }
-        if (howner) {                                                  // halo cells of this pair (x, y only)
-          double l2[2], h2[2];
-          if (two) {
-            recon_cells<RECON, 2>(G.weno_eps, u, l2, h2);
-          } else {
-            double l1[1], h1[1];
-            const double (&c1)[1][5] = reinterpret_cast<const double (&)[1][5]>(u);
-            recon_cells<RECON, 1>(G.weno_eps, c1, l1, h1);
-            l2[0] = l1[0]; h2[0] = h1[0];
-          }
+      double lo[NVR], cur[GR][5], nxt[GR][5];
+      unsigned rdy[GR];                                                // probe results for the next group's boxes
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            if (j == 0 || two) {
+      for (int j = 0; j < GR; ++j) rdy[j] = 0;
+      // reconstruct the first cnt (compile-time after unrolling) cells of u, interleaved
+      auto recon_n = [&](const double (&u)[GR][5], int cnt, double (&l)[GR], double (&h)[GR]) {
+        if (cnt >= GR) {
+          recon_cells<RECON, GR>(G.weno_eps, u, l, h);
+        } else {
+#pragma unroll
+          for (int j = 0; j < GR; ++j) {
+            if (j < cnt) {
+              double l1[1], h1[1];
+              const double (&c1)[1][5] = reinterpret_cast<const double (&)[1][5]>(u[j]);
+              recon_cells<RECON, 1>(G.weno_eps, c1, l1, h1);
+              l[j] = l1[0]; h[j] = h1[0];
+            }
+          }
+        }
+      };
+      auto fetch = [&](int v0, double (&dst)[GR][5], bool use_probe) {
+        const int cnt = (NV - v0 < GR) ? NV - v0 : GR;
+        int sj[GR];
+#pragma unroll
+        for (int j = 0; j < GR; ++j) {
+          if (j < cnt) {
+            sj[j] = st;
+            if (!(use_probe && rdy[j])) mbar_wait(&S.full[st], ph);
+            asm volatile("" ::: "memory");                             // no shared-memory load may move above the test
+            lds_stencil<RECON>(&S.ring[st][own0], sst, dst[j]);
+            if (K < 2 && warp == (v0 + j) % NWC) {                     // halo cells of this variable (x, y only)
               const int vr = v0 + j;
-              double l = l2[j], h = h2[j];
+              double u[1][5], l1[1], h1[1];
+              lds_stencil<RECON>(&S.ring[st][hal0], sst, u[0]);
+              recon_cells<RECON, 1>(G.weno_eps, u, l1, h1);
+              double l = l1[0], h = h1[0];
               if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
-                if (!(l > 0.0)) l = u[j][2];
-                if (!(h > 0.0)) h = u[j][2];
+                if (!(l > 0.0)) l = u[0][2];
+                if (!(h > 0.0)) h = u[0][2];
               }
               if (hvalid) {
                 if (hup) S.exlo[vr][hr] = l;
                 else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
               }
             }
+            if (++st == NS) { st = 0; ph ^= 1u; }
           }
         }
         // The stencils were read through the generic proxy; the refill of this stage is an async-proxy (TMA)
@@ -292,45 +298,42 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
         if (lane == 0) {
-          mbar_arrive(&S.empty[s0]);
-          if (two) mbar_arrive(&S.empty[s1]);
-        }
-        st = two ? ((s1 + 1 == NS) ? 0 : s1 + 1) : s1;
-        ph = two ? ((s1 + 1 == NS) ? p1 ^ 1u : p1) : p1;
-      };
-      auto probe = [&](int v0) {                                       // non-blocking probes of the pair at (st, ph)
-        rdy0 = mbar_test(&S.full[st], ph);
-        rdy1 = 0;
-        if (v0 + 1 < NV) {
-          const int s1 = (st + 1 == NS) ? 0 : st + 1;
-          rdy1 = mbar_test(&S.full[s1], (st + 1 == NS) ? ph ^ 1u : ph);
-        }
-      };
-      fetch(0, cur, 0u, 0u);
-      if (2 < NV) probe(2);
-      constexpr int VRAW = (((NV + 1) / 2 > 3) ? (NV + 1) / 2 - 3 : 0) * 2;   // pair at which the face metric is fetched
 #pragma unroll
-      for (int v = 0; v < NV; v += 2) {
-        if (v + 2 < NV) {
-          fetch(v + 2, nxt, rdy0, rdy1);
-          if (v + 4 < NV) probe(v + 4);
+          for (int j = 0; j < GR; ++j)
+            if (j < cnt) mbar_arrive(&S.empty[sj[j]]);
+        }
+      };
+      auto probe = [&](int v0) {                                       // non-blocking probes of the group at (st, ph)
+        int s = st;
+        unsigned p = ph;
+#pragma unroll
+        for (int j = 0; j < GR; ++j) {
+          rdy[j] = 0;
+          if (v0 + j < NV) {
+            rdy[j] = mbar_test(&S.full[s], p);
+            if (++s == NS) { s = 0; p ^= 1u; }
+          }
+        }
+      };
+      fetch(0, cur, false);
+      if (GR < NV) probe(GR);
+      constexpr int NGRP = (NV + GR - 1) / GR;
+      constexpr int VRAW = ((NGRP > 3) ? NGRP - 3 : 0) * GR;          // group at which the face metric is fetched
+#pragma unroll
+      for (int v = 0; v < NV; v += GR) {
+        if (v + GR < NV) {
+          fetch(v + GR, nxt, true);
+          if (v + 2 * GR < NV) probe(v + 2 * GR);
         }
         if (v == VRAW && solve) load_face_raw(T, K, cl, cr, raw);     // consumed after the loop
         {
-          double l2[2], h2[2];
-          if (v + 1 < NV) {
-            recon_cells<RECON, 2>(G.weno_eps, cur, l2, h2);
-          } else {
-            double l1[1], h1[1];
-            const double (&c1)[1][5] = reinterpret_cast<const double (&)[1][5]>(cur);
-            recon_cells<RECON, 1>(G.weno_eps, c1, l1, h1);
-            l2[0] = l1[0]; h2[0] = h1[0];
-          }
+          double lg[GR], hg[GR];
+          recon_n(cur, (NV - v < GR) ? NV - v : GR, lg, hg);
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
+          for (int j = 0; j < GR; ++j) {
             if (v + j < NV) {
               const int vr = v + j;
-              double l = l2[j], h = h2[j];
+              double l = lg[j], h = hg[j];
               if (vr < 2) {
                 if (!(l > 0.0)) l = cur[j][2];
                 if (!(h > 0.0)) h = cur[j][2];
@@ -342,7 +345,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           }
         }
 #pragma unroll
-        for (int j = 0; j < 2; ++j)
+        for (int j = 0; j < GR; ++j)
 #pragma unroll
           for (int q = 0; q < 5; ++q) cur[j][q] = nxt[j][q];
       }
