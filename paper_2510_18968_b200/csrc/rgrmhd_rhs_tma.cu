@@ -318,11 +318,17 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
       fetch(0, cur, false);
       if (GR < NV) probe(GR);
       constexpr int NGRP = (NV + GR - 1) / GR;
-      constexpr int VRAW = ((NGRP > 3) ? NGRP - 3 : 0) * GR;          // group at which the face metric is fetched
+      #ifndef RG_PROBE
+#define RG_PROBE true
+#endif
+#ifndef RG_VRAW_BACK
+#define RG_VRAW_BACK 3
+#endif
+      constexpr int VRAW = ((NGRP > RG_VRAW_BACK) ? NGRP - RG_VRAW_BACK : 0) * GR;          // group at which the face metric is fetched
 #pragma unroll
       for (int v = 0; v < NV; v += GR) {
         if (v + GR < NV) {
-          fetch(v + GR, nxt, true);
+          fetch(v + GR, nxt, RG_PROBE);
           if (v + 2 * GR < NV) probe(v + 2 * GR);
         }
         if (v == VRAW && solve) load_face_raw(T, K, cl, cr, raw);     // consumed after the loop
