@@ -116,6 +116,7 @@ __device__ __forceinline__ void tma_load_4d(const CUtensorMap* map, void* dst, u
 }
 // barrier among the compute warps and the edge-face warp (the producer warp never joins)
 __device__ __forceinline__ void bar_work() { asm volatile("bar.sync 1, %0;" ::"n"(NT + 32) : "memory"); }
+__device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // pin a prefetched value in its register until here (keeps the consumer arithmetic below this point)
 __device__ __forceinline__ void pin(double& x) { asm volatile("" : "+d"(x)); }
 
@@ -158,9 +159,10 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
   // producer warp: one lane walks the (plane, direction, variable) sequence NS boxes ahead
   // =================================================================================================
   if (warp == NWC) {
-    if (lane == 0) {
-      int seq = 0;
-      for (int k = k0 - 2; k < k1; ++k) {
+    int seq = 0;
+    double* const* TgtP = (STAGE == 1) ? G.Us : G.Un;
+    for (int k = k0 - 2; k < k1; ++k) {
+      if (lane == 0) {
         for (int K = (k < k0) ? 2 : 0; K < 3; ++K) {
           const CUtensorMap* map = (K == 0) ? &M.x : (K == 1) ? &M.y : &M.z;
           const unsigned bytes = 8u * (unsigned)((K == 0) ? BOX_X : (K == 1) ? BOX_Y : BOX_Z);
@@ -175,9 +177,27 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
             tma_load_4d(map, S.ring[st], &S.full[st], px, py, pz, T.fld[K][vr]);
           }
         }
+      } else {
+        // The other lanes of this warp are idle: they pull the stage-target rows and the face-metric rows of the
+        // plane after the next one into L2, so that the compute warps' loads of them two planes later are L2
+        // hits instead of DRAM accesses (no registers, no shared memory; paced by the issuing lane).
+        const int kp = k + 2;
+        if (kp >= k0 && kp < k1) {
+          const int row = (lane - 1) >> 1, half = (lane - 1) & 1;    // 31 lanes: rows 0..14 twice + row 15 once
+          for (int r = row; r < TY + 1; r += 16) {
+            if (j0 + r - 1 >= G.n[1] + 1) continue;
+            const long long cp = cell_index(G, i0 + half * 8, j0 + r - 1, kp);   // row r-1 (one halo row below the tile)
+            if (r >= 1 && r <= tyn) {
+#pragma unroll
+              for (int v = 0; v < NCONS; ++v) prefetch_l2(TgtP[v] + cp);
+            }
+#pragma unroll
+            for (int q = 0; q < 10; ++q) prefetch_l2(G.met[q] + cp);
+          }
+        }
       }
+      __syncwarp();
     }
-    __syncwarp();   // the idle lanes stay resident until the issuing lane is done
     return;
   }
 
