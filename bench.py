@@ -41,7 +41,7 @@ UNIT = "zone-cycles/s"
 # Algorithmic work of the dominant kernel (flux divergence: reconstruct + HLLE + divergence + update of the
 # stage target), per interior cell and launch -- derivation in DESIGN.md Sec. 7.
 RHS_FLOPS = {wl.RECON_WENO5: 5500.0, wl.RECON_MC: 1900.0, wl.RECON_MINMOD: 1800.0}
-RHS_DOUBLES = 55.0      # reads P 14 + jc 3 + alpha, beta, gamma_ij 10 + stage target 14, writes stage target 14
+RHS_DOUBLES = 41.0      # reads P 14 + jc 3 + alpha, beta, gamma_ij 10, writes the increment dU 14
 SRC_FLOPS = 350.0       # explicit sources + point-wise stage combine (inside the recovery kernel), per stage
 C2P_SETUP_FLOPS, C2P_EVAL_FLOPS = 250.0, 100.0   # per solve / per residual evaluation
 STEP_DOUBLES = 253.0    # algorithmic traffic of one zone-cycle

@@ -119,7 +119,7 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]);
 
 /* One IMEX-SSP2(2,2,2) step of size dt (Eq. 35-37): implicit-E + recovery (+ the point-wise
  * explicit sources and stage-combine terms of that stage), ghost fill, reconstruction + HLLE +
- * flux divergence into the stage target; twice; final recovery. */
+ * flux divergence (an increment the next recovery adds to its stage vector); twice; final recovery. */
 int rgrmhd_step(rgrmhd_t h, double dt, int scheme);
 
 /* max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k

@@ -147,7 +147,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   G.charge_mode = p->charge_mode;
   G.weno_eps = p->weno_eps > 0.0 ? p->weno_eps : 1e-26;
 
-  const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3 + rg::NSRC;
+  const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3 + rg::NSRC + rg::NCONS;
   h->field_stride = (G.ntot + 31) / 32 * 32;
   const size_t bytes = (size_t)nfields * (size_t)h->field_stride * sizeof(double);
   cudaError_t e = cudaMalloc((void**)&h->slab, bytes);
@@ -168,6 +168,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   for (int v = 0; v < rg::NCONS; ++v) G.Us[v] = next();
   for (int v = 0; v < 3; ++v) G.X1[v] = next();
   for (int v = 0; v < rg::NSRC; ++v) G.src[v] = next();
+  for (int v = 0; v < rg::NCONS; ++v) G.dU[v] = next();
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(h->slab); cudaFree(h->stats_dev); delete h; return RGRMHD_E_CUDA; }
   h->tma = rg::tma_create(G);

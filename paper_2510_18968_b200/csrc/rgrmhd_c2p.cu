@@ -270,6 +270,17 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
     double U[NCONS], P[NPRIM];
 #pragma unroll
     for (int v = 0; v < NCONS; ++v) U[v] = Ust[v][c];
+    if (STAGE != 1) {   // stage vector = bracket written by the previous recovery + increment of the flux kernel
+      double inc[NCONS];
+#pragma unroll
+      for (int v = 0; v < NCONS; ++v) inc[v] = G.dU[v][c];
+#pragma unroll
+      for (int v = 0; v < NCONS; ++v) U[v] += inc[v];
+      if (STAGE == 3) {   // U^{n+1} complete: the next step and get_cons read it from G.Un
+#pragma unroll
+        for (int v = 0; v < NCONS; ++v) Ust[v][c] = U[v];
+      }
+    }
 #pragma unroll
     for (int v = 0; v < 5; ++v) P[v] = G.P[v][c];
     const double isg = rcp_fast(sg);
@@ -299,7 +310,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
 #pragma unroll
         for (int q = 0; q < 3; ++q) cp_async8(pf + (PF_X1 + q) * NTH, G.X1[q] + c);
 #pragma unroll
-        for (int v = 0; v < NCONS; ++v) cp_async8(pf + (PF_US + v) * NTH, G.Us[v] + c);
+        for (int v = 0; v < NCONS; ++v) pf[(PF_US + v) * NTH] = U[v];   // U*2 = bracket + increment (needed again below)
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     }

@@ -45,6 +45,7 @@ struct GridView {
   double* Un[NCONS];     // U^n, overwritten with U^{n+1} by the stage-2 combine
   double* Us[NCONS];     // stage vector U*^(2)
   double* X1[3];         // calE^(1) (needed again by the final combine, Eq. 37)
+  double* dU[NCONS];     // w dt (-div F) of the last flux launch (w = 1 stage 1, 1/2 stage 2); the next recovery adds it
   double* src[NSRC];     // static source coefficients (metric derivatives, G^i, tr K; rgrmhd_sources.cuh)
   const unsigned long long* src_mask;   // device word: bit q set <=> src[q] (q < NSRC) / K_ij[q - NSRC] is not identically 0
 };

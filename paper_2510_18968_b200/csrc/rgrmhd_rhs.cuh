@@ -61,13 +61,14 @@ __device__ __forceinline__ void face_flux(const GridView& G, long long cR, doubl
 }
 
 // a5 (flux-divergence part; the point-wise part is stage_precombine in rgrmhd_sources.cuh).  dU = -div F of the
-// cell.  STAGE 1: U*2 += dt dU (G.Us);  STAGE 2: U^{n+1} += dt/2 dU (G.Un).
+// cell.  The flux kernels only WRITE the increment w dt dU (w = 1 in stage 1, 1/2 in stage 2) to G.dU; the
+// recovery kernel that follows adds it to the bracket of its stage vector (U*2 or U^{n+1}) as it loads it.  No
+// load sits in the stencil kernel's critical path and no registers are held for a read-modify-write.
 template <int STAGE>
 __device__ __forceinline__ void divergence_update(const GridView& G, long long c, double dt, const double dU[NCONS]) {
-  double* const* T = (STAGE == 1) ? G.Us : G.Un;
   const double w = (STAGE == 1) ? dt : 0.5 * dt;
 #pragma unroll
-  for (int v = 0; v < NCONS; ++v) T[v][c] += w * dU[v];
+  for (int v = 0; v < NCONS; ++v) G.dU[v][c] = w * dU[v];
 }
 
 }  // namespace rg

@@ -16,7 +16,7 @@
 //   a3  every compute thread solves the HLLE problem at its cell's lower face (x, y) / upper face (z);
 //       the TX + TY faces on the tile's upper x / y edge are solved by a helper warp, concurrently.
 //       Fluxes are exchanged through a second shared-memory buffer, so a phase needs two barriers.
-//   a5  U*2 += dt dU or U^{n+1} += dt/2 dU (one read-modify-write of the stage target, prefetched).
+//   a5  the increment dt dU or dt/2 dU is written once per cell (G.dU); the next recovery kernel adds it.
 // The face metric (two cells x 8 fields) is prefetched into registers before the reconstruction loop.
 // Warp roles: 8 compute warps, 1 producer warp (one lane issues the TMA copies), 1 edge-face warp.
 // The three directions run through ONE copy of the code (rgrmhd_flux_rot.cuh).
@@ -160,7 +160,6 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
   // =================================================================================================
   if (warp == NWC) {
     int seq = 0;
-    double* const* TgtP = (STAGE == 1) ? G.Us : G.Un;
     for (int k = k0 - 2; k < k1; ++k) {
       if (lane == 0) {
         for (int K = (k < k0) ? 2 : 0; K < 3; ++K) {
@@ -178,19 +177,15 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           }
         }
       } else {
-        // The other lanes of this warp are idle: they pull the stage-target rows and the face-metric rows of the
-        // plane after the next one into L2, so that the compute warps' loads of them two planes later are L2
-        // hits instead of DRAM accesses (no registers, no shared memory; paced by the issuing lane).
+        // The other lanes of this warp are idle: they pull the face-metric rows of the plane after the next one
+        // into L2, so that the compute warps' loads of them two planes later are L2 hits instead of DRAM
+        // accesses (no registers, no shared memory; paced by the issuing lane).
         const int kp = k + 2;
         if (kp >= k0 && kp < k1) {
           const int row = (lane - 1) >> 1, half = (lane - 1) & 1;    // 31 lanes: rows 0..14 twice + row 15 once
           for (int r = row; r < TY + 1; r += 16) {
             if (j0 + r - 1 >= G.n[1] + 1) continue;
             const long long cp = cell_index(G, i0 + half * 8, j0 + r - 1, kp);   // row r-1 (one halo row below the tile)
-            if (r >= 1 && r <= tyn) {
-#pragma unroll
-              for (int v = 0; v < NCONS; ++v) prefetch_l2(TgtP[v] + cp);
-            }
 #pragma unroll
             for (int q = 0; q < 10; ++q) prefetch_l2(G.met[q] + cp);
           }
@@ -241,7 +236,6 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
   const int hr = lane & 15;                                            // halo unit: row (x) / column (y)
   const bool hup = lane >= 16;                                         //            lower | upper halo cell
   long long c = cell_index(G, i0 + tx, j0 + ty, k0 - 2);
-  double* const* Tgt = (STAGE == 1) ? G.Us : G.Un;
   int st = 0;                                                          // ring stage of the next box to consume
   unsigned ph = 0;                                                     // and its mbarrier phase parity
   // k = k0-2: upper-face z states of plane k0-1; k = k0-1: z flux through the lower face of plane k0
@@ -375,12 +369,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
 #pragma unroll
           for (int q = 0; q < 5; ++q) cur[j][q] = nxt[j][q];
       }
-      // ---- prefetch of the stage target (z phase), consumed after the Riemann solve
-      double PLz[NVR], tgt[NCONS];
-      if (K == 2 && in && k >= k0) {
-#pragma unroll
-        for (int v = 0; v < NCONS; ++v) tgt[v] = Tgt[v][c];
-      }
+      double PLz[NVR];
       if (K < 2) bar_work();                                           // A: face states visible
       // ---- a3: HLLE at the own lower face (x, y) / upper face (z)
       double F[NCONS];
@@ -416,10 +405,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         for (int v = 0; v < NCONS; ++v) Fn[nat_z(v)] = F[v] * idz;
         if (k >= k0) {
 #pragma unroll
-          for (int v = 0; v < NCONS; ++v) {
-            pin(tgt[v]);
-            Tgt[v][c] = tgt[v] + w * (S.du[v][tid] - Fn[v]);
-          }
+          for (int v = 0; v < NCONS; ++v) G.dU[v][c] = w * (S.du[v][tid] - Fn[v]);   // a5 (divergence part), write only
         }
 #pragma unroll
         for (int v = 0; v < NCONS; ++v) S.du[v][tid] = Fn[v];          // lower z face of the next plane
