@@ -336,7 +336,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
 #define RG_PROBE true
 #endif
 #ifndef RG_VRAW_BACK
-#define RG_VRAW_BACK 3
+#define RG_VRAW_BACK 2
 #endif
       constexpr int VRAW = ((NGRP > RG_VRAW_BACK) ? NGRP - RG_VRAW_BACK : 0) * GR;          // group at which the face metric is fetched
 #pragma unroll
@@ -369,7 +369,6 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
 #pragma unroll
           for (int q = 0; q < 5; ++q) cur[j][q] = nxt[j][q];
       }
-      double PLz[NVR];
       if (K < 2) bar_work();                                           // A: face states visible
       // ---- a3: HLLE at the own lower face (x, y) / upper face (z)
       double F[NCONS];
@@ -378,13 +377,10 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         for (int q = 0; q < 8; ++q) { pin(raw.l[q]); pin(raw.r[q]); }
         FaceMet m;
         finish_face_met(raw, m);
-        {
-          const double* pl = (K == 2) ? &S.chi[(k & 1) ^ 1][0][tid] : &S.ex[0][base];
-          const int pls = (K == 2) ? NT : EXP;
-#pragma unroll
-          for (int vr = 0; vr < NV; ++vr) PLz[vr] = pl[vr * pls];
-        }
-        riemann_m<CHARGE, NV>(G, m, cl, cr, PLz, 1, lo, F);
+        // the left states are read from shared memory inside, after the right state's half of the flux
+        const double* pl = (K == 2) ? &S.chi[(k & 1) ^ 1][0][tid] : &S.ex[0][base];
+        const int pls = (K == 2) ? NT : EXP;
+        riemann_m<CHARGE, NV>(G, m, cl, cr, pl, pls, lo, F);
       }
       if (K < 2) {
         if (solve) {
