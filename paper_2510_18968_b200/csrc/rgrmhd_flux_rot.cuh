@@ -155,6 +155,33 @@ __device__ __forceinline__ void riemann_m(const GridView& G, const FaceMet& m, l
   if (NV < NVR) PL[NVR - 1] = 0.0;
   half_flux<CHARGE, false>(m, G.Gamma / (G.Gamma - 1.0), PL, sigL, wL * m.alpha, -sd - wL * m.b0, Fh);
 }
+// the same with both states in (shared) memory: right state at prp, left state at plp, each read just before
+// its half of the flux, so that only one state is live at a time
+template <int CHARGE, int NV>
+__device__ __forceinline__ void riemann_mm(const GridView& G, const FaceMet& m, long long cl, long long cr,
+                                           const double* __restrict__ plp, int pl_stride, const double* __restrict__ prp,
+                                           int pr_stride, double Fh[NCONS]) {
+  const double c = m.alpha * sqrt_fast(m.gi0[0]);
+  const double lp = fmax(0.0, c - m.b0), lm = fmin(0.0, -c - m.b0);
+  const double inv = rcp_fast(lp - lm);
+  const double wL = lp * inv, wR = -lm * inv, sd = lp * lm * inv;
+  double sigL = 0.0, sigR = 0.0;
+  if (CHARGE == CHARGE_FACE_OHM) { sigL = sigma_cell(G, cl); sigR = sigma_cell(G, cr); }
+  {
+    double PR[NVR];
+#pragma unroll
+    for (int vr = 0; vr < NV; ++vr) PR[vr] = prp[vr * pr_stride];
+    if (NV < NVR) PR[NVR - 1] = 0.0;
+    half_flux<CHARGE, true>(m, G.Gamma / (G.Gamma - 1.0), PR, sigR, wR * m.alpha, sd - wR * m.b0, Fh);
+  }
+  {
+    double PL[NVR];
+#pragma unroll
+    for (int vr = 0; vr < NV; ++vr) PL[vr] = plp[vr * pl_stride];
+    if (NV < NVR) PL[NVR - 1] = 0.0;
+    half_flux<CHARGE, false>(m, G.Gamma / (G.Gamma - 1.0), PL, sigL, wL * m.alpha, -sd - wL * m.b0, Fh);
+  }
+}
 template <int CHARGE, int NV>
 __device__ __forceinline__ void riemann(const GridView& G, const PencilTabs& T, int K, long long cl, long long cr,
                                         const double* __restrict__ plp, int pl_stride, double PR[NVR], double Fh[NCONS]) {

@@ -9,9 +9,9 @@
 // shared-memory stages.  A producer warp runs the ring ahead of the compute warps (full / empty
 // mbarriers per stage), so no compute warp ever waits on a global load for a stencil:
 //   a2  every compute thread reconstructs ITS OWN CELL along K from the staged box: the smoothness
-//       indicators are computed once and give the value at the cell's lower face (registers: the right
-//       state of that face) and at its upper face (shared memory: the left state of the neighbour's
-//       face; along z it is carried to the next plane in a thread-private slot).  The 2 x 16 halo cells
+//       indicators are computed once and give the value at the cell's lower face (a thread-private
+//       shared-memory slot: the right state of that face) and at its upper face (shared memory: the left
+//       state of the neighbour's face; along z it is carried to the next plane in a thread-private slot).  The 2 x 16 halo cells
 //       of the tile are reconstructed by one warp per variable (round robin), from the same box.
 //   a3  every compute thread solves the HLLE problem at its cell's lower face (x, y) / upper face (z);
 //       the TX + TY faces on the tile's upper x / y edge are solved by a helper warp, concurrently.
@@ -51,7 +51,8 @@ struct Smem {
   double fx[NCONS][EXP];        // face fluxes (slot = the cell whose lower face it is; column TX / row TY = edge)
   double exlo[NVR][16];         // lower-face states of the upper-halo cells (right states of the edge faces)
   double exhi[NVR][16];         // upper-face states of the last row/column (left states of the edge faces)
-  double chi[2][NVR][NT];       // z carry: upper-face states of the plane below / being reconstructed (by parity of k)
+  double chi[NVR][NT];          // z carry: upper-face states of the plane below (thread-private slots)
+  double los[NVR][NT];          // lower-face states of the own cell = right states of its face (thread-private slots)
   double du[NCONS][NT];         // flux divergence being accumulated for the current plane (thread-private)
   unsigned long long full[NS], empty[NS];
 };
@@ -255,10 +256,13 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
       const int hal0 = (K == 0) ? hr * (TX + 6) + (hup ? txn + 3 : 2) : (hup ? tyn + 3 : 2) * PY + hr + 1;
       const bool hvalid = hr < ((K == 0) ? tyn : txn);
       const bool edge = in && ((K == 0) ? (tx == txn - 1) : (K == 1) ? (ty == tyn - 1) : false);
-      double* const hi_dst = (K == 2) ? &S.chi[(k & 1)][0][tid] : &S.ex[0][base + up];
-      const int hi_str = (K == 2) ? NT : EXP;
+      // z: the new upper-face states are parked in this thread's own x slot of the (now idle) exchange buffer
+      // -- nobody else touches it between the y phase's last barrier and this thread's next x phase -- and
+      // become the carry after the Riemann solve has read the old one
+      double* const hi_dst = &S.ex[0][base + ((K == 2) ? 1 : up)];
+      const int hi_str = EXP;
       FaceRaw raw;
-      double lo[NVR], cur[GR][5], nxt[GR][5];
+      double cur[GR][5], nxt[GR][5];
       unsigned rdy[GR];                                                // probe results for the next group's boxes
 #pragma unroll
       for (int j = 0; j < GR; ++j) rdy[j] = 0;
@@ -358,7 +362,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
                 if (!(l > 0.0)) l = cur[j][2];
                 if (!(h > 0.0)) h = cur[j][2];
               }
-              lo[vr] = l;
+              S.los[vr][tid] = l;
               hi_dst[vr * hi_str] = h;
               if (edge) S.exhi[vr][(K == 0) ? ty : tx] = h;
             }
@@ -378,9 +382,9 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         FaceMet m;
         finish_face_met(raw, m);
         // the left states are read from shared memory inside, after the right state's half of the flux
-        const double* pl = (K == 2) ? &S.chi[(k & 1) ^ 1][0][tid] : &S.ex[0][base];
+        const double* pl = (K == 2) ? &S.chi[0][tid] : &S.ex[0][base];
         const int pls = (K == 2) ? NT : EXP;
-        riemann_m<CHARGE, NV>(G, m, cl, cr, pl, pls, lo, F);
+        riemann_mm<CHARGE, NV>(G, m, cl, cr, pl, pls, &S.los[0][tid], NT, F);
       }
       if (K < 2) {
         if (solve) {
@@ -405,6 +409,10 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         }
 #pragma unroll
         for (int v = 0; v < NCONS; ++v) S.du[v][tid] = Fn[v];          // lower z face of the next plane
+      }
+      if (K == 2) {                                                    // the parked upper-face states become the carry
+#pragma unroll
+        for (int vr = 0; vr < NV; ++vr) S.chi[vr][tid] = hi_dst[vr * hi_str];
       }
     }
   }
