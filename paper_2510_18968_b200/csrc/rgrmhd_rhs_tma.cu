@@ -147,7 +147,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
   const int txn = min(TX, G.n[0] - i0), tyn = min(TY, G.n[1] - j0);   // valid extent of this tile
   const int k0 = blockIdx.z * CZ, k1 = min(k0 + CZ, G.n[2]);
-  const long long sy = G.stride[1], sz = G.stride[2];
+  const long long sz = G.stride[2];
   if (tid == 0) {
 #pragma unroll
     for (int q = 0; q < NS; ++q) { mbar_init(&S.full[q], 1); mbar_init(&S.empty[q], NWC); }
