@@ -236,7 +236,7 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
 //   STAGE 2: stage vector U*2 (G.Us),       a = gamma dt; writes P, jc and the bracket of U^{n+1} into G.Un
 //   STAGE 3: recovery of U^{n+1} (G.Un) at fixed calE (a = 0, reading R12); writes P; floor write-back (R9)
 // The guess is the current G.P.  jc = undensitised conduction current of the stage (reading R3).
-constexpr int C2P_TX = 32, C2P_TY = 4;
+constexpr int C2P_TX = 32, C2P_TY = 1;
 // staging slots of the point-wise right-hand side (doubles per thread)
 enum { PF_SRC = 0, PF_K = NSRC, PF_UN = NSRC + 6, PF_X1 = NSRC + 6 + NCONS, PF_US = NSRC + 6 + NCONS + 3,
        PF_COUNT1 = PF_X1, PF_COUNT2 = PF_US + NCONS };
@@ -245,7 +245,7 @@ __device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
                : "memory");
 }
 #ifndef C2P_MINB
-#define C2P_MINB 3
+#define C2P_MINB 12
 #endif
 
 template <int STAGE>
