@@ -18,7 +18,8 @@
 //       Fluxes are exchanged through a second shared-memory buffer, so a phase needs two barriers.
 //   a5  the increment dt dU or dt/2 dU is written once per cell (G.dU); the next recovery kernel adds it.
 // The face metric (two cells x 8 fields) is prefetched into registers before the reconstruction loop.
-// Warp roles: 8 compute warps, 1 producer warp (one lane issues the TMA copies), 1 edge-face warp.
+// Warp roles: 8 compute warps, 1 producer warp (one lane issues the TMA copies), 1 edge-face warp, 2 halo
+// warps: 12 warps = three per scheduler, the most that 168 registers per thread allow.
 // The three directions run through ONE copy of the code (rgrmhd_flux_rot.cuh).
 #include <cuda.h>
 
@@ -29,7 +30,8 @@ namespace rg {
 namespace {
 constexpr int TX = 16, TY = 16, NT = TX * TY;
 constexpr int NWC = NT / 32;                       // compute warps
-constexpr int NTHREADS = NT + 64;                  // + producer warp + edge-face warp
+constexpr int NHALO = 2;                            // halo-cell warps (variables dealt round robin)
+constexpr int NTHREADS = NT + 64 + 32 * NHALO;     // + producer warp + edge-face warp + halo warps
 constexpr int EXW = TX + 1, EXH = TY + 1, EXP = EXW * EXH;
 constexpr int NS = 5;                              // ring stages
 #ifndef RG_GROUP
@@ -116,7 +118,9 @@ __device__ __forceinline__ void tma_load_4d(const CUtensorMap* map, void* dst, u
       ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
 }
 // barrier among the compute warps and the edge-face warp (the producer warp never joins)
-__device__ __forceinline__ void bar_work() { asm volatile("bar.sync 1, %0;" ::"n"(NT + 32) : "memory"); }
+__device__ __forceinline__ void bar_work() { asm volatile("bar.sync 1, %0;" ::"n"(NT + 32 + 32 * NHALO) : "memory"); }
+// barrier A ("face states visible") also has the halo warps, which write the halo states
+__device__ __forceinline__ void bar_states() { asm volatile("bar.sync 2, %0;" ::"n"(NT + 32 + 32 * NHALO) : "memory"); }
 __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // pin a prefetched value in its register until here (keeps the consumer arithmetic below this point)
 __device__ __forceinline__ void pin(double& x) { asm volatile("" : "+d"(x)); }
@@ -136,7 +140,7 @@ __device__ __forceinline__ void lds_stencil(const double* __restrict__ p, int s,
 }  // namespace
 
 template <int RECON, int CHARGE, int STAGE>
-// 168 registers: 10 warps sit 3 + 3 + 2 + 2 on the four schedulers, each with a 16 K-register file
+// 168 registers: 12 warps sit 3 + 3 + 3 + 3 on the four schedulers, each with a 16 K-register file
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTabs T,
            const __grid_constant__ TmaMaps M, double dt, int CZ) {
@@ -150,7 +154,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
   const long long sz = G.stride[2];
   if (tid == 0) {
 #pragma unroll
-    for (int q = 0; q < NS; ++q) { mbar_init(&S.full[q], 1); mbar_init(&S.empty[q], NWC); }
+    for (int q = 0; q < NS; ++q) { mbar_init(&S.full[q], 1); mbar_init(&S.empty[q], NWC + NHALO); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -210,7 +214,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         const long long cl = cr - G.stride[K];
         FaceRaw raw;
         if (valid) load_face_raw(T, K, cl, cr, raw);
-        bar_work();                                                    // A: face states visible
+        bar_states();                                                  // A: face states visible
         if (valid) {
           double PR[NVR], F[NCONS];
 #pragma unroll
@@ -223,6 +227,57 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           for (int v = 0; v < NCONS; ++v) S.fx[T.nat[K][v]][dst] = F[v];
         }
         bar_work();                                                    // C: fluxes visible
+      }
+    }
+    return;
+  }
+
+  // =================================================================================================
+  // halo warps: the 2 x 16 halo cells of the tile, one variable per warp and box (round robin); lanes 0-15 the
+  // cells below the tile (their upper-face value), lanes 16-31 the cells above (their lower-face value)
+  // =================================================================================================
+  if (warp >= NWC + 2) {
+    const int hw = warp - (NWC + 2);
+    const int hr = lane & 15;
+    const bool hup = lane >= 16;
+    int st = 0;
+    unsigned ph = 0;
+    for (int k = k0 - 2; k < k1; ++k) {
+#pragma unroll 1
+      for (int K = (k < k0) ? 2 : 0; K < 3; ++K) {
+        const int sst = (K == 0) ? 1 : PY;
+        const int hal0 = (K == 0) ? hr * (TX + 6) + (hup ? txn + 3 : 2) : (hup ? tyn + 3 : 2) * PY + hr + 1;
+        const bool hvalid = hr < ((K == 0) ? tyn : txn);
+#pragma unroll 1
+        for (int vr = 0; vr < NV; ++vr) {
+          // every consumer warp observes and releases EVERY box (an mbarrier waiter that skips a phase cannot
+          // tell it from the one two uses later); it reconstructs the halo cells only of its own variables
+          {
+            mbar_wait(&S.full[st], ph);
+            if (K < 2 && vr % NHALO == hw) {
+              double u[1][5], l1[1], h1[1];
+              lds_stencil<RECON>(&S.ring[st][hal0], sst, u[0]);
+              recon_cells<RECON, 1>(G.weno_eps, u, l1, h1);
+              double l = l1[0], h = h1[0];
+              if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
+                if (!(l > 0.0)) l = u[0][2];
+                if (!(h > 0.0)) h = u[0][2];
+              }
+              if (hvalid) {
+                if (hup) S.exlo[vr][hr] = l;
+                else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
+              }
+              asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.empty[st]);
+          }
+          if (++st == NS) { st = 0; ph ^= 1u; }
+        }
+        if (K < 2) {
+          bar_states();                                                // A: face states visible
+          bar_work();                                                  // C: every Riemann solve has read its states
+        }
       }
     }
     return;
@@ -292,21 +347,6 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
             if (!(use_probe && rdy[j])) mbar_wait(&S.full[st], ph);
             asm volatile("" ::: "memory");                             // no shared-memory load may move above the test
             lds_stencil<RECON>(&S.ring[st][own0], sst, dst[j]);
-            if (K < 2 && warp == (v0 + j) % NWC) {                     // halo cells of this variable (x, y only)
-              const int vr = v0 + j;
-              double u[1][5], l1[1], h1[1];
-              lds_stencil<RECON>(&S.ring[st][hal0], sst, u[0]);
-              recon_cells<RECON, 1>(G.weno_eps, u, l1, h1);
-              double l = l1[0], h = h1[0];
-              if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
-                if (!(l > 0.0)) l = u[0][2];
-                if (!(h > 0.0)) h = u[0][2];
-              }
-              if (hvalid) {
-                if (hup) S.exlo[vr][hr] = l;
-                else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
-              }
-            }
             if (++st == NS) { st = 0; ph ^= 1u; }
           }
         }
@@ -373,7 +413,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
 #pragma unroll
           for (int q = 0; q < 5; ++q) cur[j][q] = nxt[j][q];
       }
-      if (K < 2) bar_work();                                           // A: face states visible
+      if (K < 2) bar_states();                                         // A: face states visible
       // ---- a3: HLLE at the own lower face (x, y) / upper face (z)
       double F[NCONS];
       if (solve) {
