@@ -122,6 +122,15 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]);
  * flux divergence (an increment the next recovery adds to its stage vector); twice; final recovery. */
 int rgrmhd_step(rgrmhd_t h, double dt, int scheme);
 
+/* rgrmhd_step enqueues everything of its step except the final recovery P^{n+1} = recovery(U^{n+1}) (Eq. 37,
+ * PAPER.md:209, 242).  That launch is deferred: the next rgrmhd_step runs it inside its first recovery kernel
+ * (same arithmetic, the new state goes from one solve to the next in registers), and every entry point that reads
+ * or replaces the state or the statistics (get_*, set_*, reset_stats, this call) enqueues it first.  rgrmhd_flush
+ * enqueues it explicitly, e.g. before the end of a timed region; it does not synchronise and is a no-op when nothing
+ * is pending.  With and without deferral the same expressions are evaluated; the two compilations may contract
+ * products differently, so results agree to round-off (each call sequence on its own is deterministic). */
+int rgrmhd_flush(rgrmhd_t h);
+
 /* max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k
  * (Eq. 30); dt = CFL / that.  Synchronises. */
 int rgrmhd_max_speed(rgrmhd_t h, double* host_out);

@@ -23,7 +23,7 @@ NMETRIC = 16
 SYMBOLS = ["rgrmhd_params_default", "rgrmhd_create", "rgrmhd_destroy", "rgrmhd_set_stream", "rgrmhd_set_metric",
            "rgrmhd_set_sigma", "rgrmhd_set_prims", "rgrmhd_step", "rgrmhd_max_speed", "rgrmhd_get_prims",
            "rgrmhd_get_cons", "rgrmhd_get_stats", "rgrmhd_reset_stats", "rgrmhd_set_rhs_variant",
-           "rgrmhd_launch_count", "rgrmhd_set_timing", "rgrmhd_get_timing", "rgrmhd_measure_fp64_peak",
+           "rgrmhd_launch_count", "rgrmhd_flush", "rgrmhd_set_timing", "rgrmhd_get_timing", "rgrmhd_measure_fp64_peak",
            "rgrmhd_strerror", "rgrmhd_last_cuda_error"]
 
 KERNEL_CLASSES = ("c2p", "ghost", "rhs")
@@ -71,6 +71,7 @@ def load() -> C.CDLL:
         L.rgrmhd_get_cons.argtypes = [vp, C.POINTER(vp)]
         L.rgrmhd_get_stats.argtypes = [vp, C.POINTER(Stats)]
         L.rgrmhd_reset_stats.argtypes = [vp]
+        L.rgrmhd_flush.argtypes = [vp]
         L.rgrmhd_set_rhs_variant.argtypes = [vp, C.c_int]
         L.rgrmhd_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.rgrmhd_set_timing.argtypes = [vp, C.c_int]
@@ -208,6 +209,10 @@ class Rgrmhd:
 
     def reset_stats(self):
         self._check(self.L.rgrmhd_reset_stats(self.h), "rgrmhd_reset_stats")
+
+    def flush(self):
+        """Enqueue the deferred final recovery of the last step (no host synchronisation)."""
+        self._check(self.L.rgrmhd_flush(self.h), "rgrmhd_flush")
 
     def set_rhs_variant(self, variant: int):
         self._check(self.L.rgrmhd_set_rhs_variant(self.h, int(variant)), "rgrmhd_set_rhs_variant")

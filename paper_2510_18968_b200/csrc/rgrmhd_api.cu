@@ -6,6 +6,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <functional>
 #include <vector>
 
 #include "../../include/rgrmhd.h"
@@ -37,6 +38,7 @@ struct rgrmhd_s {
   long long solves = 0;              // host-side count of cell solves enqueued
   long long launches = 0;
   bool have_metric = false, have_prims = false, have_sigma = false;
+  bool pending_final = false;   // the last step's final recovery (k_c2p<3>) has not been launched yet
   int rhs_variant = 0;               // 0 = TMA-staged (default), 1 = simple, 2 = pencil (global-memory stencils)
   void* tma = nullptr;               // tensor maps of the TMA-staged flux kernel (null: shape not supported)
   bool timing = false;
@@ -190,8 +192,42 @@ int rgrmhd_destroy(rgrmhd_t h) {
   return RGRMHD_OK;
 }
 
+// optional per-kernel event bracket (rgrmhd_set_timing)
+static cudaError_t timed(rgrmhd_t h, int cls, const std::function<cudaError_t()>& launch) {
+  if (!h->timing) return launch();
+  rgrmhd_s::Timed t{cls, nullptr, nullptr};
+  cudaError_t e = cudaEventCreate(&t.a);
+  if (e != cudaSuccess) return e;
+  e = cudaEventCreate(&t.b);
+  if (e != cudaSuccess) { cudaEventDestroy(t.a); return e; }
+  cudaEventRecord(t.a, h->stream);
+  e = launch();
+  cudaEventRecord(t.b, h->stream);
+  h->timed.push_back(t);
+  return e;
+}
+
+// rgrmhd_step leaves the recovery of its new state (reading R12) to whoever needs that state next: the next step
+// runs it inside its first recovery kernel (k_c2p<4>), every other entry point that reads or replaces the state
+// launches it here first.
+static int finish_step(rgrmhd_t h) {
+  if (!h->pending_final) return RGRMHD_OK;
+  DeviceGuard guard(h->device);
+  RG_CUDA(h, timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(h->G, 3, 0.0, h->stats_dev, h->stream); }));
+  ++h->launches;
+  h->pending_final = false;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_flush(rgrmhd_t h) {
+  if (!h) return RGRMHD_E_INVALID;
+  return finish_step(h);
+}
+
 int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream) {
   if (!h) return RGRMHD_E_INVALID;
+  int rc;
+  if ((rc = finish_step(h))) return rc;   // on the stream the step was enqueued on
   h->stream = (cudaStream_t)cuda_stream;
   return RGRMHD_OK;
 }
@@ -218,6 +254,7 @@ int rgrmhd_set_metric(rgrmhd_t h, const double* alpha, const double* const beta[
   for (int i = 0; i < 6; ++i) if (!gam[i] || !K[i]) return RGRMHD_E_INVALID;
   DeviceGuard guard(h->device);
   int rc;
+  if ((rc = finish_step(h))) return rc;
   if ((rc = copy_in(h, h->G.met[rg::MALP], alpha))) return rc;
   for (int i = 0; i < 3; ++i) if ((rc = copy_in(h, h->G.met[rg::MBX + i], beta[i]))) return rc;
   for (int i = 0; i < 6; ++i) {
@@ -235,6 +272,7 @@ int rgrmhd_set_sigma(rgrmhd_t h, const double* sigma) {
   if (h->par.sigma_model != RGRMHD_SIGMA_ARRAY) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   int rc;
+  if ((rc = finish_step(h))) return rc;
   if ((rc = copy_in(h, h->G.sigma, sigma))) return rc;
   h->have_sigma = true;
   return RGRMHD_OK;
@@ -246,6 +284,7 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]) {
   if (!h->have_metric) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   int rc;
+  if ((rc = finish_step(h))) return rc;   // keeps the statistics complete; the state itself is replaced
   for (int v = 0; v < rg::NPRIM; ++v) if ((rc = copy_in(h, h->G.P[v], prims[v]))) return rc;
   for (int q = 0; q < 3; ++q)
     RG_CUDA(h, cudaMemsetAsync(h->G.jc[q], 0, (size_t)h->G.ntot * sizeof(double), h->stream));
@@ -277,33 +316,22 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
          : pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, st)
                   : rg::launch_rhs_simple(G, dt, stage, recon, st);
   };
-  // optional per-kernel event bracket (rgrmhd_set_timing)
-  auto timed = [&](int cls, auto&& launch) -> cudaError_t {
-    if (!h->timing) return launch();
-    rgrmhd_s::Timed t{cls, nullptr, nullptr};
-    cudaError_t e = cudaEventCreate(&t.a);
-    if (e != cudaSuccess) return e;
-    e = cudaEventCreate(&t.b);
-    if (e != cudaSuccess) { cudaEventDestroy(t.a); return e; }
-    cudaEventRecord(t.a, st);
-    e = launch();
-    cudaEventRecord(t.b, st);
-    h->timed.push_back(t);
-    return e;
-  };
   // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n.  The recovery kernel also applies the point-wise half of the
   // right-hand side (sources, implicit terms) to the stage target; the flux kernel adds -w dt div F.
-  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 1, dt, h->stats_dev, st); }));
-  if (any_active) RG_CUDA(h, timed(RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
-  RG_CUDA(h, timed(RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
+  // (if the previous step's final recovery is still due, the same kernel runs it first: k_c2p<4>)
+  const int first = h->pending_final ? 4 : 1;
+  RG_CUDA(h, timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, first, dt, h->stats_dev, st); }));
+  h->pending_final = false;
+  if (any_active) RG_CUDA(h, timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  RG_CUDA(h, timed(h, RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
   // stage 2 (Eq. 36)
-  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
-  if (any_active) RG_CUDA(h, timed(RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
-  RG_CUDA(h, timed(RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
-  // recovery of the new state at fixed calE (reading R12)
-  RG_CUDA(h, timed(RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 3, dt, h->stats_dev, st); }));
+  RG_CUDA(h, timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
+  if (any_active) RG_CUDA(h, timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  RG_CUDA(h, timed(h, RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
+  // recovery of the new state at fixed calE (reading R12): deferred, see finish_step
+  h->pending_final = true;
   h->solves += 3 * nint;
-  h->launches += 5 + (any_active ? 2 : 0);
+  h->launches += 4 + (any_active ? 2 : 0);
   return RGRMHD_OK;
 }
 
@@ -328,12 +356,13 @@ int rgrmhd_get_prims(rgrmhd_t h, double* const prims[14]) {
   for (int v = 0; v < rg::NPRIM; ++v) if (!prims[v]) return RGRMHD_E_INVALID;
   if (!h->have_prims) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
+  int rc;
+  if ((rc = finish_step(h))) return rc;
   const rg::GridView& G = h->G;
   if (G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1) {
     RG_CUDA(h, rg::launch_ghost_fill(G, G.P, rg::NPRIM, h->stream));
     ++h->launches;
   }
-  int rc;
   for (int v = 0; v < rg::NPRIM; ++v) if ((rc = copy_out(h, prims[v], G.P[v]))) return rc;
   return RGRMHD_OK;
 }
@@ -344,6 +373,7 @@ int rgrmhd_get_cons(rgrmhd_t h, double* const cons[14]) {
   if (!h->have_prims) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   int rc;
+  if ((rc = finish_step(h))) return rc;
   for (int v = 0; v < rg::NCONS; ++v) if ((rc = copy_out(h, cons[v], h->G.Un[v]))) return rc;
   return RGRMHD_OK;
 }
@@ -351,6 +381,8 @@ int rgrmhd_get_cons(rgrmhd_t h, double* const cons[14]) {
 int rgrmhd_get_stats(rgrmhd_t h, rgrmhd_stats* host_out) {
   if (!h || !host_out) return RGRMHD_E_INVALID;
   DeviceGuard guard(h->device);
+  int rc;
+  if ((rc = finish_step(h))) return rc;
   rg::StatsDev s;
   RG_CUDA(h, cudaMemcpyAsync(&s, h->stats_dev, sizeof(s), cudaMemcpyDeviceToHost, h->stream));
   RG_CUDA(h, cudaStreamSynchronize(h->stream));
@@ -366,6 +398,8 @@ int rgrmhd_get_stats(rgrmhd_t h, rgrmhd_stats* host_out) {
 int rgrmhd_reset_stats(rgrmhd_t h) {
   if (!h) return RGRMHD_E_INVALID;
   DeviceGuard guard(h->device);
+  int rc;
+  if ((rc = finish_step(h))) return rc;
   RG_CUDA(h, cudaMemsetAsync(h->stats_dev, 0, sizeof(rg::StatsDev), h->stream));
   h->solves = 0;
   return RGRMHD_OK;
@@ -381,6 +415,8 @@ int rgrmhd_get_timing(rgrmhd_t h, double ms[RGRMHD_K_COUNT], long long launches[
   if (!h || !ms || !launches) return RGRMHD_E_INVALID;
   DeviceGuard guard(h->device);
   for (int k = 0; k < RGRMHD_K_COUNT; ++k) { ms[k] = 0.0; launches[k] = 0; }
+  int rc;
+  if ((rc = finish_step(h))) return rc;
   RG_CUDA(h, cudaStreamSynchronize(h->stream));
   for (auto& t : h->timed) {
     float f = 0.f;

@@ -235,6 +235,9 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
 //   STAGE 1: stage vector U^n (X*1 = X^n),  a = gamma dt; writes P, jc, X1 and the bracket of U*2 into G.Us
 //   STAGE 2: stage vector U*2 (G.Us),       a = gamma dt; writes P, jc and the bracket of U^{n+1} into G.Un
 //   STAGE 3: recovery of U^{n+1} (G.Un) at fixed calE (a = 0, reading R12); writes P; floor write-back (R9)
+//   STAGE 4: STAGE 3 of the previous step followed by STAGE 1 of this one in the same thread (rgrmhd_step defers the
+//            final recovery until the state is asked for or the next step starts): P^{n+1} and U^{n+1} go from the
+//            first solve to the second in registers, same arithmetic as the two launches
 // The guess is the current G.P.  jc = undensitised conduction current of the stage (reading R3).
 constexpr int C2P_TX = 32, C2P_TY = 1;
 // staging slots of the point-wise right-hand side (doubles per thread)
@@ -257,7 +260,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
   const double gam = 1.0 - 0.70710678118654752440;   // 1 - 1/sqrt(2) (Eq. 35-37)
   const double adt = (STAGE == 3) ? 0.0 : gam * dt;
   double* const* Ust = (STAGE == 2) ? G.Us : G.Un;
-  int evals = 0, failed = 0, floored = 0;
+  int evals = 0, evmax = 0, failed = 0, floored = 0;
   if (i < G.n[0] && j < G.n[1]) {
     const long long c = cell_index(G, i, j, k);
     double g6[6];
@@ -276,7 +279,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       for (int v = 0; v < NCONS; ++v) inc[v] = G.dU[v][c];
 #pragma unroll
       for (int v = 0; v < NCONS; ++v) U[v] += inc[v];
-      if (STAGE == 3) {   // U^{n+1} complete: the next step and get_cons read it from G.Un
+      if (STAGE >= 3) {   // U^{n+1} complete: the next step and get_cons read it from G.Un
 #pragma unroll
         for (int v = 0; v < NCONS; ++v) Ust[v][c] = U[v];
       }
@@ -284,6 +287,27 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
 #pragma unroll
     for (int v = 0; v < 5; ++v) P[v] = G.P[v][c];
     const double isg = rcp_fast(sg);
+    if (STAGE == 4) {
+      // deferred final recovery of the previous step (a = 0): its primitives are the guess of the stage-1 solve
+      C2POut r0 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, 0.0, 0.0, G.tol, G.maxit, P);
+      evals = evmax = r0.evals; failed = r0.failed;
+      if (G.rho_floor > 0.0 && (r0.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
+        // reading R9: atmosphere reset with write-back, as in STAGE 3
+        floored = 1;
+        P[RHO] = G.rho_floor; P[VX] = P[VY] = P[VZ] = 0.0;
+        P[PRS] = G.p_atmo;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) P[EX + q] = (U[CEX + q] * isg) / (1.0 + 0.0);
+        Met m;
+        load_met_cell(G, c, m);
+        double Unew[NCONS];
+        prim2cons(m, G.Gamma, P, Unew);
+        U[CD] = Unew[CD]; U[CTAU] = Unew[CTAU];
+        Ust[CD][c] = U[CD]; Ust[CTAU][c] = U[CTAU];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) { U[CSX + q] = Unew[CSX + q]; Ust[CSX + q][c] = U[CSX + q]; }
+      }
+    }
     const double sigma = (STAGE == 3) ? 0.0 : sigma_of(G, U[CD] * isg, c);
     // The point-wise right-hand side after the solve reads ~57 more fields of this cell.  Start those loads
     // now as asynchronous copies into a thread-private shared-memory column: no registers are held and
@@ -305,7 +329,10 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
         else pf[(PF_K + q) * NTH] = 0.0;
       }
 #pragma unroll
-      for (int v = 0; v < NCONS; ++v) cp_async8(pf + (PF_UN + v) * NTH, G.Un[v] + c);
+      for (int v = 0; v < NCONS; ++v) {
+        if (STAGE == 4) pf[(PF_UN + v) * NTH] = U[v];            // U^n of this step: in registers already
+        else cp_async8(pf + (PF_UN + v) * NTH, G.Un[v] + c);
+      }
       if (STAGE == 2) {
 #pragma unroll
         for (int q = 0; q < 3; ++q) cp_async8(pf + (PF_X1 + q) * NTH, G.X1[q] + c);
@@ -315,10 +342,11 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
     C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, P);
-    evals = r2.evals; failed = r2.failed;
+    evals += r2.evals; failed += r2.failed;
+    evmax = max(evmax, r2.evals);
     if (G.rho_floor > 0.0 && (r2.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
       // reading R9: atmosphere reset
-      floored = 1;
+      floored += 1;
       P[RHO] = G.rho_floor; P[VX] = P[VY] = P[VZ] = 0.0;
       P[PRS] = G.p_atmo;
       const double s = adt * alpha * sigma;
@@ -341,7 +369,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
       sgE[q] = sg * P[EX + q];
-      if (STAGE == 1) G.X1[q][c] = sgE[q];
+      if (STAGE == 1 || STAGE == 4) G.X1[q][c] = sgE[q];
       G.jc[q][c] = (STAGE == 3) ? 0.0 : (U[CEX + q] * isg - P[EX + q]) * iada;
     }
     if (STAGE != 3) {
@@ -366,11 +394,11 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
 #pragma unroll
         for (int v = 0; v < NCONS; ++v) us[v] = pf[(PF_US + v) * NTH];
       }
-      stage_precombine<STAGE>(G, c, dt, S, sgE, un, us, x1);
+      stage_precombine<(STAGE == 4) ? 1 : STAGE>(G, c, dt, S, sgE, un, us, x1);
     }
   }
   // stats: warp reduce, one atomic per warp
-  int fl = failed, fo = floored, mx = evals;
+  int fl = failed, fo = floored, mx = evmax;
   long long ev = evals;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -454,6 +482,9 @@ cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats,
     smem = (size_t)PF_COUNT2 * C2P_TX * C2P_TY * sizeof(double);
     if ((e = cudaFuncSetAttribute(k_c2p<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
     k_c2p<2><<<grid, block, smem, st>>>(G, dt, stats);
+  } else if (stage == 4) {
+    if ((e = cudaFuncSetAttribute(k_c2p<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    k_c2p<4><<<grid, block, smem, st>>>(G, dt, stats);
   } else {
     k_c2p<3><<<grid, block, 0, st>>>(G, dt, stats);
   }

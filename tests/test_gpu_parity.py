@@ -237,6 +237,45 @@ def test_variants_agree_bitwise_or_to_roundoff(binding):
     assert e.max() <= 1e-13, e
 
 
+@pytest.mark.parametrize("which", ["blast", "tov"])
+def test_deferred_final_recovery_agrees_with_flushed(binding, which):
+    """rgrmhd_step defers its final recovery into the next step's first recovery kernel (rgrmhd.h,
+    rgrmhd_flush).  Flushing after every step (three recovery launches per step) and stepping back to
+    back (fused launch) evaluate the same expressions: agreement to round-off (the two compilations
+    contract a few products differently), identical failure / floor / solve counts, floor write-backs
+    included; each path on its own is deterministic."""
+    if which == "blast":
+        w = wl.blast_curved()
+        f, n, bc = _subblock(w, (120, 138, 100), (40, 36, 20))
+    else:
+        w = wl.tov_like()
+        i_surf = int(round((8.125 + 12.0) / w.dx[0]))
+        f, n, bc = _subblock(w, (i_surf - 20, 256 - 6, 256 - 5), (40, 12, 10))
+    out = []
+    for flush_each in (True, False, False):
+        g = binding.from_workload(w, fields=f, n=n, bc=bc)
+        l0 = g.launch_count()
+        for _ in range(6):
+            g.step(w.dt, w.recon)
+            if flush_each:
+                g.flush()
+        g.flush()
+        g.flush()                                   # nothing pending: no launch
+        nl = g.launch_count() - l0
+        out.append((interior(g.get_prims().copy(), n), interior(g.get_cons().copy(), n), g.stats(), nl))
+    (Pa, Ua, sa, la), (Pb, Ub, sb, lb), (Pc, Uc, sc, lc) = out
+    assert la == 6 * 7 and lb == 6 * 6 + 1          # 3 + 2 + 2 launches per step; one recovery fused per step pair
+    assert np.array_equal(Pb, Pc) and np.array_equal(Ub, Uc) and sb == sc      # deterministic
+    e = rel_linf(Pb, Pa, prim_group_scales(Pa, w.dx[0]))
+    assert e.max() <= 1e-13, e
+    e = rel_linf(Ub, Ua, cons_group_scales(Ua, w.dx[0]))
+    assert e.max() <= 1e-13, e
+    for k in ("c2p_solves", "c2p_failures", "floor_resets"):
+        assert sa[k] == sb[k], (sa, sb)
+    if which == "tov":
+        assert sa["floor_resets"] > 0
+
+
 def test_api_errors(binding):
     import ctypes as C
     L = binding.load()
