@@ -276,6 +276,28 @@ def test_deferred_final_recovery_agrees_with_flushed(binding, which):
         assert sa["floor_resets"] > 0
 
 
+def test_pending_recovery_and_state_replacement(binding):
+    """A step whose final recovery is still pending, followed by set_prims: the new state must not see anything of
+    the old one (same bits as a fresh handle); get_cons right after a step (no get_prims before) runs the pending
+    recovery first."""
+    w = wl.blast_curved()
+    f, n, bc = _subblock(w, (120, 138, 100), (24, 20, 12))
+    g = binding.from_workload(w, fields=f, n=n, bc=bc)
+    g.step(w.dt, w.recon)
+    U1 = interior(g.get_cons().copy(), n)                       # runs the pending recovery first
+    P1 = interior(g.get_prims().copy(), n)
+    assert np.isfinite(U1).all() and np.isfinite(P1).all()
+    g.step(w.dt, w.recon)                                       # pending again
+    g.set_prims(f["prims"])                                     # replaces the state
+    g.step(w.dt, w.recon)
+    Pa = g.get_prims().copy()
+    h = binding.from_workload(w, fields=f, n=n, bc=bc)
+    h.step(w.dt, w.recon)
+    Pb = h.get_prims().copy()
+    assert np.array_equal(interior(Pa, n), interior(Pb, n))
+    assert np.array_equal(interior(Pb, n), P1)
+
+
 def test_api_errors(binding):
     import ctypes as C
     L = binding.load()
