@@ -244,9 +244,17 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           // tell it from the one two uses later); it reconstructs the halo cells only of its own variables
           {
             mbar_wait(&S.full[st], ph);
-            if (K < 2 && vr % NHALO == hw) {
-              double u[1][5], l1[1], h1[1];
+            const bool mine = K < 2 && vr % NHALO == hw;
+            double u[1][5];
+            if (mine) {
               lds_stencil<RECON>(&S.ring[st][hal0], sst, u[0]);
+              asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            }
+            // like the compute warps: the stage goes back to the producer as soon as the stencil is in registers
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.empty[st]);
+            if (mine) {
+              double l1[1], h1[1];
               recon_cells<RECON, 1>(G.weno_eps, u, l1, h1);
               double l = l1[0], h = h1[0];
               if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
@@ -257,10 +265,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
                 if (hup) S.exlo[vr][hr] = l;
                 else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
               }
-              asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&S.empty[st]);
           }
           if (++st == NS) { st = 0; ph ^= 1u; }
         }
