@@ -33,7 +33,7 @@ constexpr int NWC = NT / 32;                       // compute warps
 constexpr int NHALO = 2;                            // halo-cell warps (variables dealt round robin)
 constexpr int NTHREADS = NT + 64 + 32 * NHALO;     // + producer warp + edge-face warp + halo warps
 constexpr int EXW = TX + 1, EXH = TY + 1, EXP = EXW * EXH;
-constexpr int NS = 5;                              // ring stages
+constexpr int NS = 6;                              // ring stages
 #ifndef RG_GROUP
 #define RG_GROUP 2
 #endif
