@@ -59,7 +59,9 @@ def lib(omp: bool = False) -> C.CDLL:
         L = C.CDLL(os.path.join(_HERE, "liboracle_omp.so" if omp else "liboracle.so"))
         L.oracle_max_speed.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
-        for name in ("oracle_prim2cons_point", "oracle_c2p_point", "oracle_c2p_literal_point",
+        L.oracle_sigma_point.restype = C.c_double
+        L.oracle_sigma_point.argtypes = [C.c_int] + [C.c_double] * 5
+        for name in ("oracle_prim2cons_point", "oracle_c2p_point", "oracle_c2p_literal_point", "oracle_c2p_plain_point",
                      "oracle_implicit_E_point", "oracle_state_flux_point", "oracle_recon_1d"):
             getattr(L, name).restype = C.c_int
         _LIBS[omp] = L
@@ -128,6 +130,10 @@ class Oracle:
         assert p.shape == (14,) + self.shape
         self._check(self.L.oracle_set_prims(self.h, _ptr_table([p[i] for i in range(14)])), "set_prims")
 
+    def set_solver(self, which: str):
+        """'plain' (default: bisection inside an un-accelerated fixed point) or 'robust' (secant + Anderson)."""
+        self._check(self.L.oracle_set_solver(self.h, {"plain": 0, "robust": 1}[which]), "set_solver")
+
     def step(self, dt: float, scheme: int):
         self._check(self.L.oracle_step(self.h, C.c_double(dt), int(scheme)), "step")
 
@@ -165,11 +171,13 @@ class Oracle:
         self.L.oracle_reset_stats(self.h)
 
 
-def from_workload(w, fields: Optional[dict] = None, omp: bool = False, n=None, bc=None, **over) -> Oracle:
+def from_workload(w, fields: Optional[dict] = None, omp: bool = False, n=None, bc=None, solver: str = "plain",
+                  **over) -> Oracle:
     """Create an oracle handle for workload `w` (or a sub-block of it) and load its fields."""
     par = w.params(n=n, bc=bc)
     par.update(over)
     o = Oracle(par, omp=omp)
+    o.set_solver(solver)
     f = fields if fields is not None else w.fields()
     o.set_metric(f["metric"])
     if f["sigma"] is not None and par["sigma_model"] == 1:
@@ -196,17 +204,25 @@ def prim2cons_point(P, gamma_eos, alpha=1.0, beta=None, g6=None):
     return U
 
 
-def c2p_point(U, guess, gamma_eos, adt=0.0, sigma=0.0, alpha=1.0, g6=None, tol=0.0, maxit=0, literal=False):
-    """Returns (prims, evals, failed)."""
+def sigma_point(model, sigma0, sigma_exp, sigma_dref, Dhat, sigma_cell=0.0):
+    return lib().oracle_sigma_point(int(model), float(sigma0), float(sigma_exp), float(sigma_dref), float(Dhat),
+                                    float(sigma_cell))
+
+
+def c2p_point(U, guess, gamma_eos, adt=0.0, sigma=0.0, alpha=1.0, g6=None, tol=0.0, maxit=0, literal=False,
+              plain=False):
+    """Returns (prims, evals, failed).  Default: the robust solver; plain=True: c2p_plain (maxit = cap on
+    outer passes); literal=True: the paper's loop."""
     P = _a(guess, 14).copy()
-    fn = lib().oracle_c2p_literal_point if literal else lib().oracle_c2p_point
+    fn = (lib().oracle_c2p_literal_point if literal else lib().oracle_c2p_plain_point if plain
+          else lib().oracle_c2p_point)
     if literal and tol <= 0:
         tol = 1e-13
     if literal and maxit <= 0:
         maxit = 100
     r = fn(C.c_double(gamma_eos), C.c_double(alpha), _dp(_a(_G_FLAT if g6 is None else g6, 6)), _dp(_a(U, 14)),
            C.c_double(adt), C.c_double(sigma), C.c_double(tol), C.c_int(maxit), _dp(P))
-    return P, abs(r), r < 0
+    return P, (r if r >= 0 else -r - 1), r < 0
 
 
 def implicit_E_point(v, s, Estar, B, alpha=1.0, g6=None, newton=False, E0=None, iters=1):

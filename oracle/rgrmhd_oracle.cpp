@@ -429,7 +429,7 @@ C2PResult c2p_robust(const Metric& m, double Gamma, const double U[NCONS], doubl
   double Z = (P[RHO] + Gamma / (Gamma - 1.0) * P[PRS]) * W * W;
   bool converged = false, state_ok = false;
   const int max_outer = 50;
-  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, slope = 1.0;
+  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, slope = 1.0, step_prev = 0.0;
   for (int outer = 0; outer < max_outer && res.evals < maxit; ++outer) {
     w.s = s0 * W; w.r = w.s / (1.0 + w.s); w.kE = kE;
     double NU[3], ND[3];
@@ -468,6 +468,10 @@ C2PResult c2p_robust(const Metric& m, double Gamma, const double U[NCONS], doubl
     const double kEnew = dotUD(w.vU, EstarD) / (1.0 + s0 * Wnew / (Wnew * Wnew));
     const bool same = std::fabs(Wnew - W) <= tol * Wnew && std::fabs(kEnew - kE) <= tol * escale;
     if (s0 == 0.0 || same) { W = Wnew; kE = kEnew; converged = true; break; }
+    // round-off stagnation (same rule as c2p_plain): the fixed-point residual has stopped shrinking below 1000 tol
+    const double step = std::max(std::fabs(Wnew - W) / Wnew, escale > 0.0 ? std::fabs(kEnew - kE) / escale : 0.0);
+    if (outer >= 2 && step >= step_prev && step <= 1000.0 * tol) { W = Wnew; kE = kEnew; converged = true; break; }
+    step_prev = step;
     // Anderson(1) acceleration of the fixed point x -> G(x), x = (W, kE/escale): with the residuals
     // f_n = G(x_n) - x_n,  x_{n+1} = G(x_n) - theta (G(x_n) - G(x_{n-1})),
     // theta = f_n.(f_n - f_{n-1}) / |f_n - f_{n-1}|^2   (the secant method when one component dominates).
@@ -495,11 +499,105 @@ C2PResult c2p_robust(const Metric& m, double Gamma, const double U[NCONS], doubl
   return res;
 }
 
+// (plain; the solver the parity runs use)  The SAME defining system as above -- Eq. 42,
+// Eq. 44-49, readings R7/R8 -- solved the dull way, so that it can be checked by eye
+// and shares no iteration logic with the CUDA kernel:
+//   outer: plain fixed point on (W, kE): freeze s = adt alpha sigma W and kE = v.E, solve the inner
+//          problem, replace (W, kE) by the values of the new v; no acceleration.  Stop when
+//          |dW| <= tol W and |d kE| <= tol |(E*^, B)|, or when the steps have stopped shrinking below
+//          1000 tol (round-off stagnation), or after `max_outer` passes (failure).
+//   inner: plain bisection of g(Z) (c2p_residual) on the rigorous bracket [D^, Gamma(tau^ + D^ - B^2/2)]
+//          (g increasing; v^2 >= 1 counts as g < 0), started from the full bracket in EVERY pass, until
+//          the bracket is <= 4 ulp wide; the midpoint of the last bracket is the root.
+// No secant, no kept slope, no safeguard logic, no Anderson mixing.  With adt = 0 or sigma = 0 the outer
+// loop is one pass.  No physical bracket (D^ <= 0 or Zhi <= Zlo): failure; rho, p, v keep the guess and
+// E is the closed form of Eq. 42 at the guess velocity.
+C2PResult c2p_plain(const Metric& m, double Gamma, const double U[NCONS], double adt, double sigma,
+                    double tol, int max_outer, double P[NPRIM] /* in: guess (v); out: primitives */) {
+  C2PWork w;
+  w.m = &m; w.Gamma = Gamma;
+  const double sg = m.sqrtg;
+  w.Dh = U[CD] / sg; w.tauh = U[CTAU] / sg;
+  const double ShD[3] = {U[CSX] / sg, U[CSY] / sg, U[CSZ] / sg};
+  double ShU[3]; raise(m, ShD, ShU);
+  double EstarD[3];
+  for (int i = 0; i < 3; ++i) { w.EstarU[i] = U[CEX + i] / sg; w.BU[i] = U[CBX + i] / sg; }
+  lower(m, w.BU, w.BD); lower(m, w.EstarU, EstarD);
+  w.B2 = dotUD(w.BU, w.BD);
+  double EsxB_U[3]; crossU(m, EstarD, w.BD, EsxB_U);
+  const double s0 = adt * m.alpha * sigma;
+  const double escale = std::sqrt(dotUD(w.EstarU, EstarD) + w.B2);
+  C2PResult res = {0, 1};
+  for (int i = 0; i < 3; ++i) P[BX + i] = w.BU[i];
+  P[PSI] = U[CPSI] / sg; P[PHI] = U[CPHI] / sg; P[QCH] = U[CQ] / sg;
+  const double Zlo = w.Dh, Zhi = Gamma * (w.tauh + w.Dh - 0.5 * w.B2);
+  // (W, kE) of the guess velocity
+  double vgU[3] = {P[VX], P[VY], P[VZ]}, vgD[3];
+  lower(m, vgU, vgD);
+  double v2g = dotUD(vgU, vgD);
+  if (!(v2g < 1.0)) { vgU[0] = vgU[1] = vgU[2] = 0; vgD[0] = vgD[1] = vgD[2] = 0; v2g = 0; }
+  double W = 1.0 / std::sqrt(1.0 - v2g);
+  double kE = dotUD(vgU, EstarD) / (1.0 + s0 * W / (W * W));
+  if (!(w.Dh > 0.0) || !(Zhi > Zlo)) {
+    implicit_E_closed(m, vgU, W, s0 * W, w.EstarU, w.BD, &P[EX]);
+    return res;
+  }
+  bool converged = false, ok = false;
+  double step_prev = 0.0;
+  for (int outer = 0; outer < max_outer; ++outer) {
+    w.s = s0 * W; w.r = w.s / (1.0 + w.s); w.kE = kE;
+    double NU[3], ND[3];
+    for (int i = 0; i < 3; ++i) NU[i] = ShU[i] - EsxB_U[i] / (1.0 + w.s);
+    lower(m, NU, ND);
+    const double NdotB = dotUD(NU, w.BD);
+    for (int i = 0; i < 3; ++i) {
+      w.NparU[i] = (w.B2 > 0.0) ? NdotB / w.B2 * w.BU[i] : 0.0;
+      w.NperpU[i] = NU[i] - w.NparU[i];
+    }
+    double NperpD[3]; lower(m, w.NperpU, NperpD);
+    crossU(m, w.BD, NperpD, w.BxNperpU);
+    // inner: bisection, invariant g(a) < 0 < g(b)
+    double a = Zlo, b = Zhi, g = 0;
+    for (;;) {
+      const double mid = 0.5 * (a + b);
+      if (!(mid > a && mid < b)) break;
+      if (b - a <= 4.0 * std::numeric_limits<double>::epsilon() * std::fabs(mid)) break;
+      const bool okm = c2p_residual(w, mid, &g); ++res.evals;
+      if (okm && g == 0.0) { a = b = mid; break; }
+      if (!okm || g < 0.0) a = mid; else b = mid;
+    }
+    ok = c2p_residual(w, 0.5 * (a + b), &g); ++res.evals;    // w now holds the state at the root
+    if (!ok) break;
+    const double Wnew = w.W;
+    const double kEnew = dotUD(w.vU, EstarD) / (1.0 + s0 * Wnew / (Wnew * Wnew));
+    // size of this pass's step, in units of the scales the tolerance refers to
+    const double step = std::max(std::fabs(Wnew - W) / Wnew, escale > 0.0 ? std::fabs(kEnew - kE) / escale : 0.0);
+    W = Wnew; kE = kEnew;
+    if (s0 == 0.0 || step <= tol) { converged = true; break; }
+    // round-off stagnation: a contraction's steps shrink until the 4-ulp noise of the inner bisection
+    // (amplified by the conditioning of strongly magnetised states) takes over; once a step is no smaller
+    // than the one before AND below 1000 tol, the fixed point has been reached as well as FP64 defines it
+    if (outer >= 2 && step >= step_prev && step <= 1000.0 * tol) { converged = true; break; }
+    step_prev = step;
+  }
+  res.failed = converged ? 0 : 1;
+  if (ok) {
+    P[RHO] = w.rho; P[PRS] = w.p;
+    for (int i = 0; i < 3; ++i) { P[VX + i] = w.vU[i]; P[EX + i] = w.EU[i]; }
+  } else {
+    implicit_E_closed(m, vgU, 1.0 / std::sqrt(1.0 - v2g), s0 / std::sqrt(1.0 - v2g), w.EstarU, w.BD, &P[EX]);
+  }
+  return res;
+}
+
 // ---------------------------------------------------------------------------------------------
 // grid container
 // ---------------------------------------------------------------------------------------------
+enum { SOLVER_PLAIN = 0, SOLVER_ROBUST = 1 };
+enum { PLAIN_MAX_OUTER = 2000 };   // passes of the un-accelerated outer fixed point before a solve counts as failed
 struct Grid {
   Params par;
+  int solver = SOLVER_PLAIN;   // which root finder solve_all uses (oracle_set_solver)
   int np[3], g[3];           // padded sizes, ghost offsets
   long ntot;
   bool have_metric = false, have_prims = false, have_sigma = false;
@@ -758,7 +856,9 @@ void solve_all(Grid& G, std::vector<double> Ust[NCONS], double adt, std::vector<
         for (int v = 0; v < NPRIM; ++v) P[v] = G.P[v][c];
         const double Dh = U[CD] / m.sqrtg;
         const double sigma = (adt > 0.0) ? sigma_of(G.par, Dh, G.have_sigma ? G.sigma[c] : 0.0) : 0.0;
-        C2PResult r = c2p_robust(m, G.par.Gamma, U, adt, sigma, G.par.c2p_tol, G.par.c2p_max_iter, P);
+        C2PResult r = (G.solver == SOLVER_PLAIN)
+                          ? c2p_plain(m, G.par.Gamma, U, adt, sigma, G.par.c2p_tol, PLAIN_MAX_OUTER, P)
+                          : c2p_robust(m, G.par.Gamma, U, adt, sigma, G.par.c2p_tol, G.par.c2p_max_iter, P);
         evals += r.evals; failures += r.failed; max_evals = std::max(max_evals, r.evals);
         if (G.par.rho_floor > 0.0 && (r.failed || !(P[RHO] > G.par.rho_floor * (1.0 + 1e-3)))) {
           // reading R9: atmosphere reset -- rho = rho_floor, v = 0, p = K rho^Gamma; E from the
@@ -971,6 +1071,16 @@ int oracle_reset_stats(void* h) {
   return 0;
 }
 
+// Which root finder the grid solves use: 0 = c2p_plain (default; bisection inside an un-accelerated fixed
+// point), 1 = c2p_robust (bracketed secant + Anderson; ~100x fewer residual evaluations; a cross-check, and
+// the only one that makes the largest multi-step parity runs finish).  Both find the root of the same system.
+int oracle_set_solver(void* h, int which) {
+  Grid* G = (Grid*)h;
+  if (!G || which < 0 || which > 1) return -1;
+  G->solver = which;
+  return 0;
+}
+
 // ---- stage-level entry points (for pins that look inside a step) ---------------------------------
 // F[U] (flux divergence + explicit sources) of the CURRENT primitives (ghosts are filled first; the
 // conduction current jc is whatever the last solve left, zero after set_prims).
@@ -999,18 +1109,31 @@ int oracle_prim2cons_point(double Gamma, double alpha, const double* beta3, cons
   prim2cons_point(m, Gamma, P, U);
   return 0;
 }
-// robust solve; P holds the guess on entry and the primitives on return.  returns evals (negative if failed)
+// robust solve; P holds the guess on entry and the primitives on return.  returns evals, or -(evals + 1) if failed
 int oracle_c2p_point(double Gamma, double alpha, const double* g6, const double* U, double adt, double sigma,
                      double tol, int maxit, double* P) {
   Metric m = metric_from_arrays(alpha, nullptr, g6);
   C2PResult r = c2p_robust(m, Gamma, U, adt, sigma, tol > 0 ? tol : 8.0 * std::ldexp(1.0, -52), maxit > 0 ? maxit : 100, P);
-  return r.failed ? -r.evals : r.evals;
+  return r.failed ? -(r.evals + 1) : r.evals;
+}
+int oracle_c2p_plain_point(double Gamma, double alpha, const double* g6, const double* U, double adt, double sigma,
+                           double tol, int max_outer, double* P) {
+  Metric m = metric_from_arrays(alpha, nullptr, g6);
+  C2PResult r = c2p_plain(m, Gamma, U, adt, sigma, tol > 0 ? tol : 8.0 * std::ldexp(1.0, -52),
+                          max_outer > 0 ? max_outer : PLAIN_MAX_OUTER, P);
+  return r.failed ? -(r.evals + 1) : r.evals;
+}
+// conductivity models at one point (A18)
+double oracle_sigma_point(int model, double sigma0, double sigma_exp, double sigma_dref, double Dhat, double sigma_cell) {
+  Params p{};
+  p.sigma_model = model; p.sigma0 = sigma0; p.sigma_exp = sigma_exp; p.sigma_dref = sigma_dref;
+  return sigma_of(p, Dhat, sigma_cell);
 }
 int oracle_c2p_literal_point(double Gamma, double alpha, const double* g6, const double* U, double adt, double sigma,
                              double tol, int maxit, double* P) {
   Metric m = metric_from_arrays(alpha, nullptr, g6);
   C2PResult r = c2p_literal(m, Gamma, U, adt, sigma, tol, maxit, P);
-  return r.failed ? -r.evals : r.evals;
+  return r.failed ? -(r.evals + 1) : r.evals;
 }
 // implicit E at fixed v: closed form (mode 0) or `iters` Newton iterations of Eq. 43 from E0 (mode 1)
 int oracle_implicit_E_point(double alpha, const double* g6, const double* vU, double s, const double* EstarU,
