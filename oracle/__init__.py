@@ -56,6 +56,9 @@ class Stats(C.Structure):
 def lib(omp: bool = False) -> C.CDLL:
     if omp not in _LIBS:
         build()
+        if omp:   # libgomp reads these when it is first loaded; an unset thread count makes it 10x slower on small grids here
+            ncpu = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+            os.environ.setdefault("OMP_NUM_THREADS", str(ncpu))
         L = C.CDLL(os.path.join(_HERE, "liboracle_omp.so" if omp else "liboracle.so"))
         L.oracle_max_speed.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
@@ -64,8 +67,15 @@ def lib(omp: bool = False) -> C.CDLL:
         for name in ("oracle_prim2cons_point", "oracle_c2p_point", "oracle_c2p_literal_point", "oracle_c2p_plain_point",
                      "oracle_implicit_E_point", "oracle_state_flux_point", "oracle_recon_1d"):
             getattr(L, name).restype = C.c_int
+        if omp:   # the cores this process may run on (a container's cpu set can be smaller than the host's count)
+            L.oracle_set_threads(len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
         _LIBS[omp] = L
     return _LIBS[omp]
+
+
+def omp_threads() -> int:
+    """Threads the OpenMP build runs on."""
+    return lib(True).oracle_set_threads(0)
 
 
 def _dp(a: Optional[np.ndarray]):
@@ -157,6 +167,21 @@ class Oracle:
         self._check(self.L.oracle_rhs(self.h, int(scheme), _ptr_table([f[i] for i in range(14)])), "rhs")
         return f
 
+    def sources(self) -> np.ndarray:
+        """Explicit sources S of the current primitives (interior cells; ghosts of the result are zero)."""
+        f = np.zeros((14,) + self.shape)
+        self._check(self.L.oracle_sources(self.h, _ptr_table([f[i] for i in range(14)])), "sources")
+        return f
+
+    def face_states(self, scheme: int, d: int, i: int, j: int = 0, k: int = 0):
+        """(PL, PR, fixups) at the lower face in direction d of interior cell (i, j, k); fills the ghosts first."""
+        self.get_prims()
+        PL, PR = np.empty(14), np.empty(14)
+        r = self.L.oracle_face_states(self.h, int(scheme), int(d), int(i), int(j), int(k), _dp(PL), _dp(PR))
+        if r < 0:
+            raise RuntimeError("face_states failed")
+        return PL, PR, r
+
     def ghost_fill(self, field: np.ndarray) -> np.ndarray:
         f = np.ascontiguousarray(field, dtype=np.float64).copy()
         self._check(self.L.oracle_ghost_fill(self.h, _dp(f)), "ghost_fill")
@@ -165,7 +190,9 @@ class Oracle:
     def stats(self) -> dict:
         s = Stats()
         self._check(self.L.oracle_get_stats(self.h, C.byref(s)), "get_stats")
-        return {k: getattr(s, k) for k, _ in Stats._fields_ if k != "reserved"}
+        d = {k: getattr(s, k) for k, _ in Stats._fields_ if k != "reserved"}
+        d["face_fixups"] = s.reserved      # reading R4 fix-ups (rho/p fallbacks + |v| limiter hits) of the RHS evaluations
+        return d
 
     def reset_stats(self):
         self.L.oracle_reset_stats(self.h)

@@ -31,6 +31,9 @@
 #include <cstring>
 #include <limits>
 #include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 namespace {
 
@@ -608,7 +611,7 @@ struct Grid {
   std::vector<double> X1[3], X2[3];                  // stage electric fields calE^(1), calE^(2)
   std::vector<double> Xs2[3];                        // calE*^(2)
   // stats
-  long long solves = 0, evals = 0, failures = 0, floors = 0; int max_evals = 0;
+  long long solves = 0, evals = 0, failures = 0, floors = 0, face_fixups = 0; int max_evals = 0;
 
   long idx(int i, int j, int k) const { return (long)(i + g[0]) + (long)np[0] * ((long)(j + g[1]) + (long)np[1] * (long)(k + g[2])); }
   bool active(int d) const { return par.n[d] > 1; }
@@ -671,7 +674,7 @@ void ghost_fill_field(const Grid& G, std::vector<double>& f) {
 //   PAPER.md:171-173, Eq. 30 (reading R6: lambda+- = +-alpha sqrt(gamma^kk) - beta^k, clipped)
 // ---------------------------------------------------------------------------------------------
 void face_state(const Grid& G, int scheme, int d, int i, int j, int k, int which /*0: at -1/2, 1: at +1/2*/,
-                double Pf[NPRIM], double* jck) {
+                double Pf[NPRIM], double* jck, int* fixups) {
   int o[3] = {0, 0, 0}; o[d] = 1;
   long c[5];
   for (int q = -2; q <= 2; ++q) c[q + 2] = G.idx(i + q * o[0], j + q * o[1], k + q * o[2]);
@@ -683,26 +686,35 @@ void face_state(const Grid& G, int scheme, int d, int i, int j, int k, int which
     if (v < NPRIM) Pf[v] = val; else *jck = val;
   }
   // reading R4: unphysical face values fall back to the cell value
-  if (!(Pf[RHO] > 0.0)) Pf[RHO] = G.P[RHO][c[2]];
-  if (!(Pf[PRS] > 0.0)) Pf[PRS] = G.P[PRS][c[2]];
+  if (!(Pf[RHO] > 0.0)) { Pf[RHO] = G.P[RHO][c[2]]; ++*fixups; }
+  if (!(Pf[PRS] > 0.0)) { Pf[PRS] = G.P[PRS][c[2]]; ++*fixups; }
 }
 
-void hlle_face(const Grid& G, int scheme, int d, int i, int j, int k, double Fh[NCONS]) {
+// the two states of the Riemann problem at the lower face (index -1/2 in direction d) of cell (i,j,k), after the
+// fix-ups of reading R4 (rho, p fallback above; |v| limited with the FACE metric mf); returns the number of fix-ups
+int face_states(const Grid& G, int scheme, int d, int i, int j, int k, const Metric& mf, double PL[NPRIM],
+                double PR[NPRIM], double* jL, double* jR) {
   int o[3] = {0, 0, 0}; o[d] = 1;
-  const int il = i - o[0], jl = j - o[1], kl = k - o[2];
-  const long cL = G.idx(il, jl, kl), cR = G.idx(i, j, k);
-  Metric mf; metric_face(G, cL, cR, mf);
-  double PL[NPRIM], PR[NPRIM], jL, jR;
-  face_state(G, scheme, d, il, jl, kl, 1, PL, &jL);      // left cell's value at its +1/2 face
-  face_state(G, scheme, d, i, j, k, 0, PR, &jR);         // right cell's value at its -1/2 face
-  // reading R4: limit |v| with the face metric
+  int fixups = 0;
+  face_state(G, scheme, d, i - o[0], j - o[1], k - o[2], 1, PL, jL, &fixups);      // left cell's value at its +1/2 face
+  face_state(G, scheme, d, i, j, k, 0, PR, jR, &fixups);                          // right cell's value at its -1/2 face
   double* Ps[2] = {PL, PR};
   for (int sd = 0; sd < 2; ++sd) {
     double vU[3] = {Ps[sd][VX], Ps[sd][VY], Ps[sd][VZ]}, vD[3];
     lower(mf, vU, vD);
     const double v2 = dotUD(vU, vD), v2max = 1.0 - 1e-10;
-    if (v2 >= v2max) { const double f = std::sqrt(v2max / v2); for (int q = 0; q < 3; ++q) Ps[sd][VX + q] *= f; }
+    if (v2 >= v2max) { const double f = std::sqrt(v2max / v2); for (int q = 0; q < 3; ++q) Ps[sd][VX + q] *= f; ++fixups; }
   }
+  return fixups;
+}
+
+int hlle_face(const Grid& G, int scheme, int d, int i, int j, int k, double Fh[NCONS]) {
+  int o[3] = {0, 0, 0}; o[d] = 1;
+  const int il = i - o[0], jl = j - o[1], kl = k - o[2];
+  const long cL = G.idx(il, jl, kl), cR = G.idx(i, j, k);
+  Metric mf; metric_face(G, cL, cR, mf);
+  double PL[NPRIM], PR[NPRIM], jL, jR;
+  const int fixups = face_states(G, scheme, d, i, j, k, mf, PL, PR, &jL, &jR);
   double sigL = 0, sigR = 0;
   if (G.par.charge_mode == CHARGE_FACE_OHM) {            // reading R6b: piecewise-constant sigma
     Metric mL, mR; metric_at(G, cL, mL); metric_at(G, cR, mR);
@@ -723,6 +735,7 @@ void hlle_face(const Grid& G, int scheme, int d, int i, int j, int k, double Fh[
   const double lp = std::max(0.0, c - mf.betaU[d]);
   const double lm = std::min(0.0, -c - mf.betaU[d]);
   for (int v = 0; v < NCONS; ++v) Fh[v] = (lp * FL[v] - lm * FR[v] + lp * lm * (UR[v] - UL[v])) / (lp - lm);
+  return fixups;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -804,20 +817,21 @@ void rhs_all(Grid& G, int scheme, std::vector<double> Fout[NCONS]) {
   for (int v = 0; v < NCONS; ++v) std::fill(Fout[v].begin(), Fout[v].end(), 0.0);
   std::vector<double> Fh[NCONS];
   for (int v = 0; v < NCONS; ++v) Fh[v].assign(G.ntot, 0.0);
+  long long fixups = 0;
   for (int d = 0; d < 3; ++d) {
     if (!G.active(d)) continue;
     int o[3] = {0, 0, 0}; o[d] = 1;
     // faces at the lower side of cells 0..n (inclusive) in direction d
-#pragma omp parallel for collapse(2) schedule(static)
+#pragma omp parallel for collapse(3) schedule(static) reduction(+ : fixups)
     for (int k = 0; k < nz + o[2]; ++k)
       for (int j = 0; j < ny + o[1]; ++j)
         for (int i = 0; i < nx + o[0]; ++i) {
           double f[NCONS];
-          hlle_face(G, scheme, d, i, j, k, f);
+          fixups += hlle_face(G, scheme, d, i, j, k, f);
           const long c = G.idx(i, j, k);
           for (int v = 0; v < NCONS; ++v) Fh[v][c] = f[v];
         }
-#pragma omp parallel for collapse(2) schedule(static)
+#pragma omp parallel for collapse(3) schedule(static)
     for (int k = 0; k < nz; ++k)
       for (int j = 0; j < ny; ++j)
         for (int i = 0; i < nx; ++i) {
@@ -825,7 +839,7 @@ void rhs_all(Grid& G, int scheme, std::vector<double> Fout[NCONS]) {
           for (int v = 0; v < NCONS; ++v) Fout[v][c] -= (Fh[v][cp] - Fh[v][c]) / G.par.dx[d];
         }
   }
-#pragma omp parallel for collapse(2) schedule(static)
+#pragma omp parallel for collapse(3) schedule(static)
   for (int k = 0; k < nz; ++k)
     for (int j = 0; j < ny; ++j)
       for (int i = 0; i < nx; ++i) {
@@ -834,6 +848,7 @@ void rhs_all(Grid& G, int scheme, std::vector<double> Fout[NCONS]) {
         const long c = G.idx(i, j, k);
         for (int v = 0; v < NCONS; ++v) Fout[v][c] += S[v];
       }
+  G.face_fixups += fixups;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -845,7 +860,7 @@ void rhs_all(Grid& G, int scheme, std::vector<double> Fout[NCONS]) {
 void solve_all(Grid& G, std::vector<double> Ust[NCONS], double adt, std::vector<double>* Xout, bool write_back_floor) {
   const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2];
   long long evals = 0, failures = 0, floors = 0; int max_evals = 0;
-#pragma omp parallel for collapse(2) schedule(static) reduction(+ : evals, failures, floors) reduction(max : max_evals)
+#pragma omp parallel for collapse(3) schedule(static) reduction(+ : evals, failures, floors) reduction(max : max_evals)
   for (int k = 0; k < nz; ++k)
     for (int j = 0; j < ny; ++j)
       for (int i = 0; i < nx; ++i) {
@@ -902,6 +917,7 @@ void step(Grid& G, double dt, int scheme) {
   for (int q = 0; q < 3; ++q) ghost_fill_field(G, G.jc[q]);
   rhs_all(G, scheme, G.F1);
   // stage 2 (Eq. 36)
+#pragma omp parallel for collapse(3) schedule(static)
   for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
     const long c = G.idx(i, j, k);
     for (int v = 0; v < NCONS; ++v) G.Us[v][c] = G.Un[v][c] + dt * G.F1[v][c];
@@ -916,6 +932,7 @@ void step(Grid& G, double dt, int scheme) {
   for (int q = 0; q < 3; ++q) ghost_fill_field(G, G.jc[q]);
   rhs_all(G, scheme, G.F2);
   // final combination (Eq. 37)
+#pragma omp parallel for collapse(3) schedule(static)
   for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
     const long c = G.idx(i, j, k);
     double Unew[NCONS];
@@ -1061,13 +1078,13 @@ int oracle_get_stats(void* h, oracle_stats* s) {
   Grid* G = (Grid*)h;
   if (!G || !s) return -1;
   s->c2p_solves = G->solves; s->c2p_evals = G->evals; s->c2p_failures = G->failures; s->floor_resets = G->floors;
-  s->c2p_max_evals = G->max_evals; s->reserved = 0;
+  s->c2p_max_evals = G->max_evals; s->reserved = (int)std::min<long long>(G->face_fixups, 2147483647LL);
   return 0;
 }
 int oracle_reset_stats(void* h) {
   Grid* G = (Grid*)h;
   if (!G) return -1;
-  G->solves = G->evals = G->failures = G->floors = 0; G->max_evals = 0;
+  G->solves = G->evals = G->failures = G->floors = G->face_fixups = 0; G->max_evals = 0;
   return 0;
 }
 
@@ -1092,6 +1109,27 @@ int oracle_rhs(void* h, int scheme, double* const out[14]) {
   rhs_all(*G, scheme & 0xff, G->F1);
   for (int v = 0; v < NCONS; ++v) std::copy(G->F1[v].begin(), G->F1[v].end(), out[v]);
   return 0;
+}
+// explicit sources S (a4, second half) of the CURRENT primitives alone, no flux divergence
+int oracle_sources(void* h, double* const out[14]) {
+  Grid* G = (Grid*)h;
+  if (!G || !out) return -1;
+  for (int k = 0; k < G->par.n[2]; ++k) for (int j = 0; j < G->par.n[1]; ++j) for (int i = 0; i < G->par.n[0]; ++i) {
+    double S[NCONS];
+    sources_cell(*G, i, j, k, S);
+    for (int v = 0; v < NCONS; ++v) out[v][G->idx(i, j, k)] = S[v];
+  }
+  return 0;
+}
+// the two reconstructed states (after the fix-ups of reading R4) at the lower face, in direction d, of cell (i,j,k)
+// of the CURRENT primitives (ghosts must be filled: call oracle_get_prims or oracle_rhs first); returns the fix-up count
+int oracle_face_states(void* h, int scheme, int d, int i, int j, int k, double* PL, double* PR) {
+  Grid* G = (Grid*)h;
+  if (!G || !PL || !PR || d < 0 || d > 2) return -1;
+  int o[3] = {0, 0, 0}; o[d] = 1;
+  Metric mf; metric_face(*G, G->idx(i - o[0], j - o[1], k - o[2]), G->idx(i, j, k), mf);
+  double jL, jR;
+  return face_states(*G, scheme & 0xff, d, i, j, k, mf, PL, PR, &jL, &jR);
 }
 int oracle_ghost_fill(void* h, double* field) {
   Grid* G = (Grid*)h;
@@ -1157,6 +1195,16 @@ int oracle_state_flux_point(double Gamma, double alpha, const double* beta3, con
 int oracle_recon_1d(int scheme, double eps_w, int n, const double* u, double* at_minus, double* at_plus) {
   for (int i = 2; i < n - 2; ++i) recon_cell(scheme, eps_w > 0 ? eps_w : 1e-26, u[i - 2], u[i - 1], u[i], u[i + 1], u[i + 2], &at_minus[i], &at_plus[i]);
   return 0;
+}
+// number of OpenMP threads of the -fopenmp build (no effect on results: cells are independent, max is exact)
+int oracle_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+  return omp_get_max_threads();
+#else
+  (void)n;
+  return 1;
+#endif
 }
 int oracle_omp_enabled(void) {
 #ifdef _OPENMP

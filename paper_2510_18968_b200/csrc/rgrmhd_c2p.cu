@@ -71,7 +71,7 @@ __device__ __forceinline__ void implicit_E_closed(const double v[3], double W, d
 // P holds the guess (rho, p, v^i) on entry and all 14 primitives on return.  sg = sqrt(gamma).
 __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double alpha, double Gamma, double gog1,
                                             double gm1og, const double U[NCONS], double adt, double sigma, double tol,
-                                            int maxit, double P[NPRIM]) {
+                                            int maxit, unsigned lanes, double P[NPRIM]) {
   const double Dh = U[CD] * isg, tauh = U[CTAU] * isg;
   double Sh[3], Es[3], B[3], EsxB[3];
   triad_from_cov(t, U[CSX] * isg, U[CSY] * isg, U[CSZ] * isg, Sh);
@@ -110,7 +110,7 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
   const int max_outer = 50;
   // inverse slope of g for the first secant step: dg/dZ ~ 1 - (Gamma-1)/Gamma / W^2 at fixed v (exact in the
   // unmagnetised, slow limit), instead of 1
-  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, islope = rcp_fast(1.0 - gm1og * (1.0 - v2g));
+  double fW_prev = 0, fk_prev = 0, GW_prev = 0, Gk_prev = 0, step_prev = 0, islope = rcp_fast(1.0 - gm1og * (1.0 - v2g));
   // frozen per outer pass
   double s = 0, r = 0, i1s = 1, Npar[3] = {0, 0, 0}, Nperp[3] = {0, 0, 0}, BxN[3] = {0, 0, 0};
   // last evaluation
@@ -188,7 +188,11 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
           const double Wnew = Wv;
           const double kEnew = dot3(v, Es) * Wnew * rcp_fast(Wnew + s0);
           const bool same = fabs(Wnew - W) <= tol * Wnew && fabs(kEnew - kE) <= tol * escale;
-          if (s0 == 0.0 || same) {
+          // round-off stagnation: the fixed-point residual no longer shrinks and is below 1000 tol
+          const double step = fmax(fabs(Wnew - W) * rcp_fast(Wnew), fabs(kEnew - kE) * ies);
+          const bool stalled = outer >= 2 && step >= step_prev && step <= 1000.0 * tol;
+          step_prev = step;
+          if (s0 == 0.0 || same || stalled) {
             converged = true; done = true;
           } else {
             // Anderson(1) acceleration of x -> G(x), x = (W, kE/escale)
@@ -211,7 +215,7 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
         }
       }
     }
-    if (__all_sync(__activemask(), done)) break;            // warp-vote exit
+    if (__all_sync(lanes, done)) break;                     // warp-vote exit over the lanes that entered the solve
   }
   res.failed = converged ? 0 : 1;
   double EU[3];
@@ -261,7 +265,9 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
   const double adt = (STAGE == 3) ? 0.0 : gam * dt;
   double* const* Ust = (STAGE == 2) ? G.Us : G.Un;
   int evals = 0, evmax = 0, failed = 0, floored = 0;
-  if (i < G.n[0] && j < G.n[1]) {
+  const bool in_range = i < G.n[0] && j < G.n[1];
+  const unsigned lanes = __ballot_sync(0xffffffffu, in_range);   // the lanes that take part in the solver's warp votes
+  if (in_range) {
     const long long c = cell_index(G, i, j, k);
     double g6[6];
 #pragma unroll
@@ -289,7 +295,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
     const double isg = rcp_fast(sg);
     if (STAGE == 4) {
       // deferred final recovery of the previous step (a = 0): its primitives are the guess of the stage-1 solve
-      C2POut r0 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, 0.0, 0.0, G.tol, G.maxit, P);
+      C2POut r0 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, 0.0, 0.0, G.tol, G.maxit, lanes, P);
       evals = evmax = r0.evals; failed = r0.failed;
       if (G.rho_floor > 0.0 && (r0.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
         // reading R9: atmosphere reset with write-back, as in STAGE 3
@@ -341,7 +347,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
-    C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, P);
+    C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, lanes, P);
     evals += r2.evals; failed += r2.failed;
     evmax = max(evmax, r2.evals);
     if (G.rho_floor > 0.0 && (r2.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {

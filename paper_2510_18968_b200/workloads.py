@@ -15,6 +15,9 @@ DESIGN.md "Input recipe"):
   cfg3  3D rotated CP Alfven wave         (Eq. 56-59)
   cfg4  3D blast in a static curved metric(PAPER.md:303-321 relative, curved metric)
   cfg5  3D TOV-like magnetised star       (Eq. 60)
+and the paper's own tests that BASELINE.json does not list:
+  e2    1D shocktube, sigma = sigma0 D^gamma (Eq. 51-52)
+  e3    2D cylindrical explosion 200^2      (Eq. 53)
 
 Layout: every field is a padded array of shape (nzp, nyp, nxp) (x fastest), where
 n?p = n? + 2*ng for an active direction (n? > 1) and 1 for an inactive one.
@@ -339,8 +342,22 @@ def _gen_tov(w: Workload, X, Y, Z, I, J, K, full):
     return P, metric, None
 
 
+def _gen_explosion2d(w: Workload, X, Y, Z, I, J, K, full):
+    """Eq. 53: rho_in inside r_in, rho_out outside r_out, log-linear ramp between (the pressure
+    likewise); uniform B^x; everything else zero."""
+    e = w.extra
+    z = np.zeros(full)
+    r = np.sqrt(X * X + Y * Y) + z
+    t = np.clip((r - e["r_in"]) / (e["r_out"] - e["r_in"]), 0.0, 1.0)
+    P = [z.copy() for _ in range(NPRIM)]
+    P[RHO] = np.exp((1.0 - t) * math.log(e["rho_in"]) + t * math.log(e["rho_out"]))
+    P[PRS] = np.exp((1.0 - t) * math.log(e["p_in"]) + t * math.log(e["p_out"]))
+    P[BX] = z + e["Bx"]
+    return P, _flat_metric(full), None
+
+
 _GENERATORS = {"shocktube": _gen_shocktube, "current_sheet": _gen_current_sheet,
-               "alfven": _gen_alfven, "blast": _gen_blast, "tov": _gen_tov}
+               "alfven": _gen_alfven, "blast": _gen_blast, "tov": _gen_tov, "explosion2d": _gen_explosion2d}
 
 
 # ------------------------------------------------------------------------------------------
@@ -359,6 +376,30 @@ def shocktube(n=400, sigma0=1e6, recon=RECON_WENO5, cfl=0.4, axis=0, t_end=0.4,
                  (BC_OUTFLOW,) * 3, gamma_eos, recon, cfl, 0,
                  sigma_model=SIGMA_UNIFORM, sigma0=sigma0,
                  extra=dict(kind="shocktube", left=left, right=right))
+    w.nsteps = int(round(t_end / w.dt))
+    return w
+
+
+def shocktube_paper(n=400, sigma0=1e6, gamma_exp=0, recon=RECON_MINMOD, cfl=0.25, t_end=0.4) -> Workload:
+    """The paper's own shocktube (Eq. 51): B = (0, +-0.5, 0), Gamma = 2, minmod, CFL 0.25, x in
+    [-0.5, 0.5]; conductivity sigma0 D^gamma_exp (Eq. 52; gamma_exp = 0 is the uniform case, the paper runs 0, 6, 9, 12
+    at sigma0 = 1e6 and dx = 0.0025)."""
+    w = shocktube(n=n, sigma0=sigma0, recon=recon, cfl=cfl, t_end=t_end,
+                  left=dict(rho=1.0, p=1.0, By=0.5), right=dict(rho=0.125, p=0.1, By=-0.5))
+    w.name = "e2_shocktube_sigmaD%d" % gamma_exp
+    if gamma_exp:
+        w.sigma_model, w.sigma_exp, w.sigma_dref = SIGMA_POWER_D, float(gamma_exp), 1.0
+    return w
+
+
+def explosion2d(n=200, sigma0=1e6, recon=RECON_MINMOD, cfl=0.25, t_end=4.0) -> Workload:
+    """The paper's 2D cylindrical explosion (Eq. 53): n x n cells on [-6, 6]^2, Gamma = 4/3,
+    outflow, uniform sigma; rho_in = 0.01, p_in = 1 inside r = 0.8, rho_out = p_out = 1e-3 outside r = 1, B^x = 0.05."""
+    dx = 12.0 / n
+    w = Workload("e3_explosion2d", (n, n, 1), (dx, dx, dx), (-6.0, -6.0, 0.0), (BC_OUTFLOW,) * 3, 4.0 / 3.0,
+                 recon, cfl, 0, sigma_model=SIGMA_UNIFORM, sigma0=sigma0,
+                 extra=dict(kind="explosion2d", r_in=0.8, r_out=1.0, rho_in=0.01, p_in=1.0, rho_out=1e-3, p_out=1e-3,
+                            Bx=0.05))
     w.nsteps = int(round(t_end / w.dt))
     return w
 
@@ -431,7 +472,7 @@ def tov_like(n=512, recon=RECON_WENO5, cfl=0.125, nsteps=10, seed=5) -> Workload
 
 
 CONFIGS = {"cfg1": shocktube, "cfg2": current_sheet, "cfg3": alfven3d,
-           "cfg4": blast_curved, "cfg5": tov_like}
+           "cfg4": blast_curved, "cfg5": tov_like, "e2": shocktube_paper, "e3": explosion2d}
 
 
 def get(name: str, **kw) -> Workload:

@@ -1,0 +1,206 @@
+"""GPU parity tests (-m gpu) for the code paths round 1 left unreached: the conductivity models ATMO (Eq. 61) and
+POWER_D with exponents other than 2 (Eq. 52; the paper's own shocktube E2), the 2D explosion E3, the atmosphere rule
+(reading R9) against hand-typed values through both recovery routes, max speed with a shift, and the face fix-ups
+(reading R4).  Everything goes through the C-ABI binding; expected values come from the oracle or from closed forms."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from helpers import cons_group_scales, interior, prim_group_scales, rel_linf
+from paper_2510_18968_b200 import workloads as wl
+from test_oracle_closed_forms import fixup_stencil_prims, floor_hand_case, shifted_diagonal_metric
+
+pytestmark = pytest.mark.gpu
+
+TOL1, TOL20 = 1e-11, 1e-9
+
+
+@pytest.fixture(scope="module")
+def binding():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2510_18968_b200 import binding as b
+    b.load()
+    return b
+
+
+def _compare(g, o, n, dx_min, tol, what=""):
+    Pg, Po = interior(g.get_prims(), n), interior(o.get_prims(), n)
+    Ug, Uo = interior(g.get_cons(), n), interior(o.get_cons(), n)
+    assert np.isfinite(Pg).all() and np.isfinite(Ug).all(), what
+    eP = rel_linf(Pg, Po, prim_group_scales(Po, dx_min))
+    eU = rel_linf(Ug, Uo, cons_group_scales(Uo, dx_min))
+    assert eP.max() <= tol and eU.max() <= tol, (what, eP, eU)
+    return max(eP.max(), eU.max())
+
+
+def _both(binding, par, metric, prims, variant=0, omp=True):
+    o = oracle.Oracle(par, omp=omp)
+    g = binding.Rgrmhd(par)
+    g.set_rhs_variant(variant)
+    for h in (o, g):
+        h.set_metric(metric); h.set_prims(prims)
+    return g, o
+
+
+# ----------------------------------------------------------------------------------------------
+# conductivity models
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gamma_exp", [6, 12])
+def test_e2_shocktube_power_law_conductivity(binding, gamma_exp):
+    """The paper's E2: sigma = 1e6 D^gamma, 400 cells, minmod; sigma spans ~12 decades."""
+    w = wl.shocktube_paper(gamma_exp=gamma_exp)
+    f = w.fields()
+    g = binding.from_workload(w, fields=f)
+    o = oracle.from_workload(w, fields=f)
+    for s in range(20):
+        g.step(w.dt, w.recon); o.step(w.dt, w.recon)
+        if s == 0:
+            _compare(g, o, w.n, w.dx[0], TOL1, "e2 step 1")
+    _compare(g, o, w.n, w.dx[0], TOL20, "e2 step 20")
+    assert g.stats()["c2p_failures"] == 0 and o.stats()["c2p_failures"] == 0
+
+
+def test_e2_shocktube_to_t04(binding):
+    """E2 with gamma = 6 in full: 640 steps to t = 0.4 (bound: the 20-step one scaled linearly, as for config 1)."""
+    w = wl.shocktube_paper(gamma_exp=6)
+    f = w.fields()
+    g = binding.from_workload(w, fields=f)
+    o = oracle.from_workload(w, fields=f)
+    for _ in range(w.nsteps):
+        g.step(w.dt, w.recon); o.step(w.dt, w.recon)
+    _compare(g, o, w.n, w.dx[0], (w.nsteps / 20) * TOL20, "e2 t=0.4")
+    # the conductivity really is non-uniform: sigma0 D^6 spans many decades across the tube
+    D = interior(g.get_cons(), w.n)[0]
+    assert (D.max() / D.min()) ** 6 > 1e4
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_sigma_atmo_model_tov_subblock(binding, variant):
+    """Eq. 61: sigma = sigma0 max(1 - D_atmo/D, 0)^2 on a block across the stellar surface of the
+    config-5 star: zero conductivity in the atmosphere, sigma0 inside."""
+    w = wl.tov_like()
+    i_surf = int(round((8.125 + 12.0) / w.dx[0]))
+    n, bc = (40, 12, 10), (wl.BC_OUTFLOW,) * 3
+    f = w.fields((i_surf - 20, 256 - 6, 256 - 5), n)
+    over = dict(sigma_model=wl.SIGMA_ATMO, sigma0=1e6, sigma_dref=1e-10)
+    o = oracle.from_workload(w, fields=f, omp=True, n=n, bc=bc, **over)
+    g = binding.from_workload(w, fields=f, n=n, bc=bc, **over)
+    g.set_rhs_variant(variant)
+    for s in range(10):
+        g.step(w.dt, w.recon); o.step(w.dt, w.recon)
+        if s == 0:
+            _compare(g, o, n, w.dx[0], TOL1, "atmo step 1")
+    _compare(g, o, n, w.dx[0], TOL20, "atmo step 10")
+    sg, so = g.stats(), o.stats()
+    assert sg["floor_resets"] == so["floor_resets"] > 0 and sg["c2p_failures"] == so["c2p_failures"] == 0
+
+
+def test_sigma_atmo_model_face_ohm(binding):
+    """The same model through charge mode A, where the flux kernel itself evaluates sigma(D) of the two cells."""
+    rng = np.random.default_rng(5)
+    from test_oracle_scheme import _pad_periodic, _periodic_problem
+    n = (20, 10, 8)
+    metric, P = _periodic_problem(24, rng, True)
+    sl = (slice(None), slice(0, n[2]), slice(0, n[1]), slice(0, n[0]))
+    metric, P = _pad_periodic(np.ascontiguousarray(metric[sl])), _pad_periodic(np.ascontiguousarray(P[sl]))
+    for model, extra in ((wl.SIGMA_ATMO, dict(sigma0=40.0, sigma_dref=0.95)),
+                         (wl.SIGMA_POWER_D, dict(sigma0=25.0, sigma_exp=3.0, sigma_dref=1.1))):
+        par = dict(n=n, dx=(1 / 24,) * 3, bc=(0, 0, 0), gamma_eos=5 / 3, sigma_model=model, kappa=1.0,
+                   charge_mode=wl.CHARGE_FACE_OHM, **extra)
+        for variant in (0, 1):
+            g, o = _both(binding, par, metric, P, variant)
+            for _ in range(3):
+                g.step(0.2 / 24, wl.RECON_MC); o.step(0.2 / 24, wl.RECON_MC)
+            _compare(g, o, n, 1 / 24, TOL20, "face-ohm sigma model %d" % model)
+
+
+# ----------------------------------------------------------------------------------------------
+# E3: the paper's 2D cylindrical explosion
+# ----------------------------------------------------------------------------------------------
+def test_e3_explosion2d_full_200x200(binding):
+    w = wl.explosion2d()
+    f = w.fields()
+    g = binding.from_workload(w, fields=f)
+    o = oracle.from_workload(w, fields=f, omp=True)
+    for s in range(20):
+        g.step(w.dt, w.recon); o.step(w.dt, w.recon)
+        if s == 0:
+            _compare(g, o, w.n, w.dx[0], TOL1, "e3 step 1")
+    _compare(g, o, w.n, w.dx[0], TOL20, "e3 step 20")
+    assert g.stats()["c2p_failures"] == 0
+
+
+# ----------------------------------------------------------------------------------------------
+# atmosphere rule against hand-typed values, both recovery routes
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("route", ["flushed", "fused"])
+def test_floor_rule_hand_case_gpu(binding, route):
+    """tests/test_oracle_closed_forms.floor_hand_case: the expected primitives AND the written-back D, S_i, tau are
+    typed by hand there.  'flushed' runs the final recovery as its own launch (k_c2p<3>) after every step, 'fused'
+    lets the next step's first launch do it (k_c2p<4>)."""
+    par, m, P, dt, expect, (lo, hi) = floor_hand_case()
+    g = binding.Rgrmhd(par)
+    g.set_metric(m); g.set_prims(P)
+    for nsteps in (1, 2):
+        g.step(dt, wl.RECON_WENO5)
+        if route == "flushed" or nsteps == 2:
+            g.flush()
+        if route == "fused" and nsteps == 1:
+            continue                                            # keep the recovery pending: step 2 fuses it
+        Pg = interior(g.get_prims(), par["n"])[:, 0, 0, :]
+        Ug = interior(g.get_cons(), par["n"])[:, 0, 0, :]
+        prim, cons = expect(nsteps)
+        for f in range(14):
+            assert np.allclose(Pg[f, lo], prim[f], rtol=1e-13, atol=1e-18), (route, nsteps, f, Pg[f, lo], prim[f])
+            assert np.allclose(Ug[f, lo], cons[f], rtol=1e-13, atol=1e-18), (route, nsteps, f, Ug[f, lo], cons[f])
+        Pi = interior(P, par["n"])[:, 0, 0, :]
+        assert np.allclose(Pg[:, hi], Pi[:, hi], rtol=1e-12, atol=1e-16)       # above the threshold: untouched
+    st = g.stats()
+    assert st["c2p_failures"] == 0 and st["floor_resets"] >= 3 * 2 * 12
+
+
+# ----------------------------------------------------------------------------------------------
+# a7 with a shift
+# ----------------------------------------------------------------------------------------------
+def test_max_speed_with_shift_gpu(binding):
+    n, dx = (37, 21, 9), (0.1, 0.2, 0.15)
+    par = dict(n=n, dx=dx, bc=(1, 1, 1), gamma_eos=2.0)
+    g = binding.Rgrmhd(par)
+    m = shifted_diagonal_metric(g.shape, n, dx)
+    g.set_metric(m)
+    mi = interior(m, n)
+    exp = max(np.max((mi[0] / np.sqrt(mi[q]) + np.abs(mi[1 + k])) / dx[k]) for k, q in enumerate((4, 7, 9)))
+    o = oracle.Oracle(par)
+    o.set_metric(m)
+    assert g.max_speed() == pytest.approx(exp, rel=1e-14)
+    assert abs(g.max_speed() - o.max_speed()) <= 1e-15 * exp
+    m0 = m.copy(); m0[1:4] = 0
+    g.set_metric(m0)
+    assert g.max_speed() < 0.95 * exp                              # the |beta^k| term is live
+
+
+# ----------------------------------------------------------------------------------------------
+# face fix-ups
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_face_fixup_stencil(binding, variant):
+    """A profile on which WENO5 undershoots below zero in rho and p (tests/test_oracle_closed_forms pins the oracle's
+    fallback values): 1D, and replicated along y and z so that the tiled kernels and their halo warps take the same
+    decision; a wrong or missing fallback changes the fluxes at O(1)."""
+    P1 = fixup_stencil_prims()
+    for n in ((24, 1, 1), (24, 18, 6)):
+        shape = tuple(m + 6 if m > 1 else 1 for m in (n[2], n[1], n[0]))
+        P = np.ascontiguousarray(np.broadcast_to(P1, (14,) + shape[:2] + (30,)))
+        m = np.zeros((16,) + shape); m[0] = 1.0; m[4] = m[7] = m[9] = 1.0
+        par = dict(n=n, dx=(0.1, 0.1, 0.1), bc=(1, 1, 1), gamma_eos=5 / 3, sigma0=10.0)
+        g, o = _both(binding, par, m, P, variant)
+        dt = 0.02
+        g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+        assert o.stats()["face_fixups"] > 0
+        _compare(g, o, n, 0.1, TOL1, "fix-up stencil n=%s" % (n,))
+        for _ in range(4):
+            g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+        _compare(g, o, n, 0.1, TOL20, "fix-up stencil 5 steps n=%s" % (n,))
