@@ -12,8 +12,8 @@
  * covariant; gamma_ij, K_ij covariant, stored xx,xy,xz,yy,yz,zz.
  *
  * Pointers: every field pointer may be a DEVICE pointer on params.device or a HOST pointer
- * (pageable or pinned); the library classifies it with cudaPointerGetAttributes and issues
- * the matching stream-ordered copy.  Pointer tables (the `const double* const x[14]`
+ * (pageable or pinned); the library copies with cudaMemcpyAsync(..., cudaMemcpyDefault) on its
+ * stream, so unified addressing classifies the pointer.  Pointer tables (the `const double* const x[14]`
  * arguments) are HOST arrays of such pointers.  Host scalars/structs are written
  * synchronously.
  *
@@ -42,7 +42,9 @@ typedef struct rgrmhd_s* rgrmhd_t;
 enum rgrmhd_status {
   RGRMHD_OK        =  0,
   RGRMHD_E_INVALID = -1, /* null pointer, ng != 3, n < 1, dx <= 0, Gamma <= 1, unknown enum     */
-  RGRMHD_E_STATE   = -2, /* step/get before set_metric + set_prims; set_sigma w/o ARRAY model  */
+  RGRMHD_E_STATE   = -2, /* step/get before set_metric + set_prims; set_sigma w/o ARRAY model;
+                            any call but set_prims/destroy after a launch inside rgrmhd_step failed
+                            (the state is half advanced: the handle refuses to hand it out)      */
   RGRMHD_E_CUDA    = -3, /* a CUDA call failed; rgrmhd_last_cuda_error() returns its string    */
   RGRMHD_E_NOMEM   = -4  /* device allocation failed                                            */
 };
@@ -102,7 +104,10 @@ int rgrmhd_params_default(rgrmhd_params* p);
 int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p);
 int rgrmhd_destroy(rgrmhd_t h);
 
-/* Use `cuda_stream` (a cudaStream_t, e.g. torch's current stream) for all later work. */
+/* Use `cuda_stream` (a cudaStream_t, e.g. torch's current stream) for all later work.  Work already enqueued
+ * on the previous stream (copies of set_*, kernels, a pending final recovery -- which is flushed there first) is
+ * ordered BEFORE anything enqueued later on the new stream (event on the old stream, wait on the new one), so the
+ * switch is safe between any two calls, also with non-blocking streams. */
 int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream);
 
 /* Fixed 3+1 metric: lapse, shift beta^i, gamma_ij, K_ij as padded
@@ -151,6 +156,9 @@ int rgrmhd_reset_stats(rgrmhd_t h);
  * direction); 2 = the pencil-tiled kernel that reads its stencils straight from global memory.  All
  * implement the same arithmetic and agree to rounding. */
 int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant);
+/* The variant the last rgrmhd_step actually launched (before any step: the one the next step would launch), which
+ * differs from the requested one when the block shape forces a fallback. */
+int rgrmhd_get_rhs_variant(rgrmhd_t h, int* host_out);
 
 /* Kernel launches enqueued by this handle since create (bench.py's "gpu_launches"). */
 int rgrmhd_launch_count(rgrmhd_t h, long long* host_out);

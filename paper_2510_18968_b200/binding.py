@@ -22,7 +22,7 @@ NMETRIC = 16
 
 SYMBOLS = ["rgrmhd_params_default", "rgrmhd_create", "rgrmhd_destroy", "rgrmhd_set_stream", "rgrmhd_set_metric",
            "rgrmhd_set_sigma", "rgrmhd_set_prims", "rgrmhd_step", "rgrmhd_max_speed", "rgrmhd_get_prims",
-           "rgrmhd_get_cons", "rgrmhd_get_stats", "rgrmhd_reset_stats", "rgrmhd_set_rhs_variant",
+           "rgrmhd_get_cons", "rgrmhd_get_stats", "rgrmhd_reset_stats", "rgrmhd_set_rhs_variant", "rgrmhd_get_rhs_variant",
            "rgrmhd_launch_count", "rgrmhd_flush", "rgrmhd_set_timing", "rgrmhd_get_timing", "rgrmhd_measure_fp64_peak",
            "rgrmhd_strerror", "rgrmhd_last_cuda_error"]
 
@@ -73,6 +73,7 @@ def load() -> C.CDLL:
         L.rgrmhd_reset_stats.argtypes = [vp]
         L.rgrmhd_flush.argtypes = [vp]
         L.rgrmhd_set_rhs_variant.argtypes = [vp, C.c_int]
+        L.rgrmhd_get_rhs_variant.argtypes = [vp, C.POINTER(C.c_int)]
         L.rgrmhd_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.rgrmhd_set_timing.argtypes = [vp, C.c_int]
         L.rgrmhd_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
@@ -216,6 +217,11 @@ class Rgrmhd:
 
     def set_rhs_variant(self, variant: int):
         self._check(self.L.rgrmhd_set_rhs_variant(self.h, int(variant)), "rgrmhd_set_rhs_variant")
+
+    def get_rhs_variant(self) -> int:
+        out = C.c_int()
+        self._check(self.L.rgrmhd_get_rhs_variant(self.h, C.byref(out)), "rgrmhd_get_rhs_variant")
+        return out.value
 
     def set_timing(self, enable: bool):
         self._check(self.L.rgrmhd_set_timing(self.h, int(bool(enable))), "rgrmhd_set_timing")

@@ -17,13 +17,13 @@ cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats,
 cudaError_t launch_prim2cons(const GridView& G, cudaStream_t st);
 cudaError_t launch_metric_coeffs(const GridView& G, cudaStream_t st);
 cudaError_t launch_rhs_simple(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
-cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
+cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, int sm_count, cudaStream_t st);
 bool rhs_pencil_supported(const GridView& G);
-cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int stage, int recon, cudaStream_t st);
+cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int stage, int recon, int sm_count, cudaStream_t st);
 void* tma_create(const GridView& G);
 void tma_destroy(void* state);
 cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, cudaStream_t st);
-cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, cudaStream_t st);
+cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, int sm_count, cudaStream_t st);
 }  // namespace rg
 
 struct rgrmhd_s {
@@ -39,6 +39,9 @@ struct rgrmhd_s {
   long long launches = 0;
   bool have_metric = false, have_prims = false, have_sigma = false;
   bool pending_final = false;   // the last step's final recovery (k_c2p<3>) has not been launched yet
+  bool poisoned = false;        // a launch inside rgrmhd_step failed: the state is half advanced until set_prims replaces it
+  int sm_count = 148;           // multiprocessors of the device (grid sizing of the flux and reduction kernels)
+  int last_rhs_variant = -1;    // flux kernel the last rgrmhd_step actually launched
   int rhs_variant = 0;               // 0 = TMA-staged (default), 1 = simple, 2 = pencil (global-memory stencils)
   void* tma = nullptr;               // tensor maps of the TMA-staged flux kernel (null: shape not supported)
   bool timing = false;
@@ -157,8 +160,10 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   e = cudaMalloc((void**)&h->stats_dev, sizeof(rg::StatsDev) + 2 * sizeof(unsigned long long));
   if (e != cudaSuccess) { cudaGetLastError(); cudaFree(h->slab); delete h; return RGRMHD_E_NOMEM; }
   h->maxspeed_dev = (unsigned long long*)(h->stats_dev + 1);
-  cudaMemset(h->slab, 0, bytes);
-  cudaMemset(h->stats_dev, 0, sizeof(rg::StatsDev) + 2 * sizeof(unsigned long long));
+  e = cudaMemset(h->slab, 0, bytes);
+  if (e == cudaSuccess) e = cudaMemset(h->stats_dev, 0, sizeof(rg::StatsDev) + 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device);
+  if (e != cudaSuccess) { cudaGetLastError(); cudaFree(h->slab); cudaFree(h->stats_dev); delete h; return RGRMHD_E_CUDA; }
   G.src_mask = h->maxspeed_dev + 1;
   double* q = h->slab;
   auto next = [&]() { double* r = q; q += h->field_stride; return r; };
@@ -193,6 +198,7 @@ int rgrmhd_destroy(rgrmhd_t h) {
 }
 
 // optional per-kernel event bracket (rgrmhd_set_timing)
+static const size_t kMaxTimed = 1 << 16;
 static cudaError_t timed(rgrmhd_t h, int cls, const std::function<cudaError_t()>& launch) {
   if (!h->timing) return launch();
   rgrmhd_s::Timed t{cls, nullptr, nullptr};
@@ -200,9 +206,14 @@ static cudaError_t timed(rgrmhd_t h, int cls, const std::function<cudaError_t()>
   if (e != cudaSuccess) return e;
   e = cudaEventCreate(&t.b);
   if (e != cudaSuccess) { cudaEventDestroy(t.a); return e; }
-  cudaEventRecord(t.a, h->stream);
-  e = launch();
-  cudaEventRecord(t.b, h->stream);
+  e = cudaEventRecord(t.a, h->stream);
+  if (e == cudaSuccess) e = launch();
+  if (e == cudaSuccess) e = cudaEventRecord(t.b, h->stream);
+  if (e != cudaSuccess) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); return e; }
+  if (h->timed.size() >= kMaxTimed) {   // nobody collects them (rgrmhd_get_timing): drop the oldest bracket
+    cudaEventDestroy(h->timed.front().a); cudaEventDestroy(h->timed.front().b);
+    h->timed.erase(h->timed.begin());
+  }
   h->timed.push_back(t);
   return e;
 }
@@ -211,9 +222,11 @@ static cudaError_t timed(rgrmhd_t h, int cls, const std::function<cudaError_t()>
 // runs it inside its first recovery kernel (k_c2p<4>), every other entry point that reads or replaces the state
 // launches it here first.
 static int finish_step(rgrmhd_t h) {
+  if (h->poisoned) return RGRMHD_E_STATE;
   if (!h->pending_final) return RGRMHD_OK;
   DeviceGuard guard(h->device);
-  RG_CUDA(h, timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(h->G, 3, 0.0, h->stats_dev, h->stream); }));
+  const cudaError_t e = timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(h->G, 3, 0.0, h->stats_dev, h->stream); });
+  if (e != cudaSuccess) { h->poisoned = true; return fail_cuda(h, e, "launch_c2p(final recovery)"); }
   ++h->launches;
   h->pending_final = false;
   return RGRMHD_OK;
@@ -226,15 +239,35 @@ int rgrmhd_flush(rgrmhd_t h) {
 
 int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream) {
   if (!h) return RGRMHD_E_INVALID;
+  DeviceGuard guard(h->device);
   int rc;
-  if ((rc = finish_step(h))) return rc;   // on the stream the step was enqueued on
-  h->stream = (cudaStream_t)cuda_stream;
+  if (!h->poisoned && (rc = finish_step(h))) return rc;   // on the stream the step was enqueued on
+  const cudaStream_t next = (cudaStream_t)cuda_stream;
+  if (next != h->stream) {
+    // everything already enqueued on the old stream (copies of set_*, kernels, the recovery just flushed) must be
+    // complete before later work on the new stream touches the state: event on the old, wait on the new
+    cudaEvent_t ev;
+    RG_CUDA(h, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    cudaError_t e = cudaEventRecord(ev, h->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(next, ev, 0);
+    cudaEventDestroy(ev);                                  // released once the recorded work has completed
+    if (e != cudaSuccess) return fail_cuda(h, e, "stream hand-over");
+    h->stream = next;
+  }
   return RGRMHD_OK;
 }
 
 int rgrmhd_set_rhs_variant(rgrmhd_t h, int variant) {
   if (!h || variant < 0 || variant > 2) return RGRMHD_E_INVALID;
   h->rhs_variant = variant;
+  return RGRMHD_OK;
+}
+
+int rgrmhd_get_rhs_variant(rgrmhd_t h, int* host_out) {
+  if (!h || !host_out) return RGRMHD_E_INVALID;
+  if (h->last_rhs_variant >= 0) { *host_out = h->last_rhs_variant; return RGRMHD_OK; }
+  const bool tma = h->rhs_variant == 0 && h->tma != nullptr;
+  *host_out = tma ? 0 : (h->rhs_variant != 1 && rg::rhs_pencil_supported(h->G)) ? 2 : 1;
   return RGRMHD_OK;
 }
 
@@ -284,6 +317,7 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]) {
   if (!h->have_metric) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   int rc;
+  if (h->poisoned) { h->poisoned = false; h->pending_final = false; }   // the half-advanced state is replaced below
   if ((rc = finish_step(h))) return rc;   // keeps the statistics complete; the state itself is replaced
   for (int v = 0; v < rg::NPRIM; ++v) if ((rc = copy_in(h, h->G.P[v], prims[v]))) return rc;
   for (int q = 0; q < 3; ++q)
@@ -298,7 +332,7 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   if (!h || !(dt > 0.0)) return RGRMHD_E_INVALID;
   const int recon = scheme & RGRMHD_RECON_MASK;
   if (recon > RGRMHD_RECON_WENO5 || (scheme & ~RGRMHD_RECON_MASK) != RGRMHD_TIME_IMEX_SSP2_222) return RGRMHD_E_INVALID;
-  if (!h->have_metric || !h->have_prims || (h->par.sigma_model == RGRMHD_SIGMA_ARRAY && !h->have_sigma))
+  if (!h->have_metric || !h->have_prims || (h->par.sigma_model == RGRMHD_SIGMA_ARRAY && !h->have_sigma) || h->poisoned)
     return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   const rg::GridView& G = h->G;
@@ -312,22 +346,31 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   const bool tma = h->rhs_variant == 0 && h->tma != nullptr;
   const bool pencil = !tma && h->rhs_variant != 1 && rg::rhs_pencil_supported(G);
   auto rhs = [&](int stage) {
-    return tma    ? rg::launch_rhs_tma(G, h->tma, dt, stage, recon, st)
-         : pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, st)
+    return tma    ? rg::launch_rhs_tma(G, h->tma, dt, stage, recon, h->sm_count, st)
+         : pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, h->sm_count, st)
                   : rg::launch_rhs_simple(G, dt, stage, recon, st);
   };
   // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n.  The recovery kernel also applies the point-wise half of the
   // right-hand side (sources, implicit terms) to the stage target; the flux kernel adds -w dt div F.
   // (if the previous step's final recovery is still due, the same kernel runs it first: k_c2p<4>)
   const int first = h->pending_final ? 4 : 1;
-  RG_CUDA(h, timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, first, dt, h->stats_dev, st); }));
+  h->last_rhs_variant = tma ? 0 : pencil ? 2 : 1;
+  // From the first launch on the state is in flight: if any launch fails, the handle is marked poisoned and every
+  // later call but set_prims / destroy returns RGRMHD_E_STATE (the state is half advanced, nothing can read it safely).
+#define RG_STEP(call)                                                              \
+  do {                                                                             \
+    cudaError_t e__ = (call);                                                      \
+    if (e__ != cudaSuccess) { h->poisoned = true; h->pending_final = false; return fail_cuda(h, e__, #call); } \
+  } while (0)
+  RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, first, dt, h->stats_dev, st); }));
   h->pending_final = false;
-  if (any_active) RG_CUDA(h, timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
-  RG_CUDA(h, timed(h, RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
+  if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
   // stage 2 (Eq. 36)
-  RG_CUDA(h, timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
-  if (any_active) RG_CUDA(h, timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
-  RG_CUDA(h, timed(h, RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
+  RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
+  if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
+#undef RG_STEP
   // recovery of the new state at fixed calE (reading R12): deferred, see finish_step
   h->pending_final = true;
   h->solves += 3 * nint;
@@ -340,7 +383,7 @@ int rgrmhd_max_speed(rgrmhd_t h, double* host_out) {
   if (!h->have_metric) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   RG_CUDA(h, cudaMemsetAsync(h->maxspeed_dev, 0, sizeof(unsigned long long), h->stream));
-  RG_CUDA(h, rg::launch_max_speed(h->G, h->maxspeed_dev, h->stream));
+  RG_CUDA(h, rg::launch_max_speed(h->G, h->maxspeed_dev, h->sm_count, h->stream));
   ++h->launches;
   unsigned long long bits = 0;
   RG_CUDA(h, cudaMemcpyAsync(&bits, h->maxspeed_dev, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
@@ -448,14 +491,15 @@ int rgrmhd_measure_fp64_peak(int device, int repeats, double* tflops_out) {
   double* out = nullptr;
   if (cudaMalloc((void**)&out, sizeof(double)) != cudaSuccess) return RGRMHD_E_NOMEM;
   cudaEvent_t a, b;
-  cudaEventCreate(&a); cudaEventCreate(&b);
+  if (cudaEventCreate(&a) != cudaSuccess) { cudaFree(out); return RGRMHD_E_CUDA; }
+  if (cudaEventCreate(&b) != cudaSuccess) { cudaEventDestroy(a); cudaFree(out); return RGRMHD_E_CUDA; }
   const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 1 << 14;
   double best = 0.0;
   for (int r = 0; r < repeats + 1; ++r) {
     cudaEventRecord(a);
     k_dfma_peak<<<blocks, threads>>>(out, iters, 0.999999, 1e-9);
     cudaEventRecord(b);
-    if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(out); return RGRMHD_E_CUDA; }
+    if (cudaEventSynchronize(b) != cudaSuccess) { cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(out); return RGRMHD_E_CUDA; }
     float ms = 0.f;
     cudaEventElapsedTime(&ms, a, b);
     const double tf = 2.0 * 8.0 * (double)iters * blocks * threads / (ms * 1e-3) * 1e-12;
@@ -477,7 +521,7 @@ const char* rgrmhd_strerror(int code) {
   switch (code) {
     case RGRMHD_OK: return "ok";
     case RGRMHD_E_INVALID: return "invalid argument";
-    case RGRMHD_E_STATE: return "call out of order (metric / primitives / sigma not set, or wrong sigma model)";
+    case RGRMHD_E_STATE: return "call out of order (metric / primitives / sigma not set, wrong sigma model, or a failed step left the state unusable until set_prims)";
     case RGRMHD_E_CUDA: return "CUDA error (see rgrmhd_last_cuda_error)";
     case RGRMHD_E_NOMEM: return "device allocation failed";
   }

@@ -14,7 +14,7 @@
 //       and its neighbour's flux.  No face is solved twice except the TX + TY faces on the tile's
 //       upper x / y edge, which one warp each handles in an extra pass (their reconstruction halo:
 //       two more partial warps).
-//   a5  U*2 += dt dU or U^{n+1} += dt/2 dU (one read-modify-write of the stage target).
+//   a5  the increment dt dU or dt/2 dU is written once per cell (G.dU, write only); the next recovery kernel adds it.
 // The three directions run through ONE copy of the reconstruction and Riemann code: direction K is a
 // run-time cyclic rotation of the vector/tensor components (cyclic permutations keep the Levi-Civita
 // sign, so Eq. 27 is form invariant), realised for free as index arithmetic on pointer tables and
@@ -219,17 +219,17 @@ bool rhs_pencil_supported(const GridView& G) {
   return G.n[0] > 1 && G.n[1] > 1 && G.n[2] > 1;
 }
 
-static int choose_cz(const GridView& G) {
-  // several waves of 148 SMs x 2 CTAs, but long enough pencils to amortise the two lead-in planes
+static int choose_cz(const GridView& G, int sm_count) {
+  // several waves of (SM count) x 2 CTAs, but long enough pencils to amortise the two lead-in planes
   const long long tiles = (long long)((G.n[0] + TX - 1) / TX) * ((G.n[1] + TY - 1) / TY);
   int cz = 64;
-  while (cz > 8 && tiles * ((G.n[2] + cz - 1) / cz) < 148LL * 2 * 4) cz /= 2;
+  while (cz > 8 && tiles * ((G.n[2] + cz - 1) / cz) < (long long)sm_count * 2 * 4) cz /= 2;
   return cz;
 }
 
 template <int RECON, int CHARGE, int STAGE>
-static cudaError_t launch_one(const GridView& G, double dt, cudaStream_t st) {
-  const int cz = choose_cz(G);
+static cudaError_t launch_one(const GridView& G, double dt, int sm_count, cudaStream_t st) {
+  const int cz = choose_cz(G, sm_count);
   const PencilTabs T = make_tabs(G);
   dim3 block(TX, TY, 1);
   dim3 grid((G.n[0] + TX - 1) / TX, (G.n[1] + TY - 1) / TY, (G.n[2] + cz - 1) / cz);
@@ -241,22 +241,22 @@ static cudaError_t launch_one(const GridView& G, double dt, cudaStream_t st) {
 }
 
 template <int RECON, int CHARGE>
-static cudaError_t launch_rc(const GridView& G, double dt, int stage, cudaStream_t st) {
-  return stage == 1 ? launch_one<RECON, CHARGE, 1>(G, dt, st) : launch_one<RECON, CHARGE, 2>(G, dt, st);
+static cudaError_t launch_rc(const GridView& G, double dt, int stage, int sm_count, cudaStream_t st) {
+  return stage == 1 ? launch_one<RECON, CHARGE, 1>(G, dt, sm_count, st) : launch_one<RECON, CHARGE, 2>(G, dt, sm_count, st);
 }
 
-cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, cudaStream_t st) {
+cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, int sm_count, cudaStream_t st) {
   const bool ohm = G.charge_mode == CHARGE_FACE_OHM;
   switch (recon) {
     case RECON_MINMOD:
-      return ohm ? launch_rc<RECON_MINMOD, CHARGE_FACE_OHM>(G, dt, stage, st)
-                 : launch_rc<RECON_MINMOD, CHARGE_CELL_CURRENT>(G, dt, stage, st);
+      return ohm ? launch_rc<RECON_MINMOD, CHARGE_FACE_OHM>(G, dt, stage, sm_count, st)
+                 : launch_rc<RECON_MINMOD, CHARGE_CELL_CURRENT>(G, dt, stage, sm_count, st);
     case RECON_MC:
-      return ohm ? launch_rc<RECON_MC, CHARGE_FACE_OHM>(G, dt, stage, st)
-                 : launch_rc<RECON_MC, CHARGE_CELL_CURRENT>(G, dt, stage, st);
+      return ohm ? launch_rc<RECON_MC, CHARGE_FACE_OHM>(G, dt, stage, sm_count, st)
+                 : launch_rc<RECON_MC, CHARGE_CELL_CURRENT>(G, dt, stage, sm_count, st);
     default:
-      return ohm ? launch_rc<RECON_WENO5, CHARGE_FACE_OHM>(G, dt, stage, st)
-                 : launch_rc<RECON_WENO5, CHARGE_CELL_CURRENT>(G, dt, stage, st);
+      return ohm ? launch_rc<RECON_WENO5, CHARGE_FACE_OHM>(G, dt, stage, sm_count, st)
+                 : launch_rc<RECON_WENO5, CHARGE_CELL_CURRENT>(G, dt, stage, sm_count, st);
   }
 }
 

@@ -171,11 +171,11 @@ k_max_speed(const __grid_constant__ GridView G, unsigned long long* __restrict__
   }
 }
 
-cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, cudaStream_t st) {
+cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, int sm_count, cudaStream_t st) {
   const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
   const int threads = 256;
   long long blocks = (nint + threads - 1) / threads;
-  if (blocks > 148 * 8) blocks = 148 * 8;
+  if (blocks > (long long)sm_count * 8) blocks = (long long)sm_count * 8;   // 8 resident 256-thread CTAs per SM
   k_max_speed<<<(unsigned)blocks, threads, 0, st>>>(G, out);
   return cudaGetLastError();
 }

@@ -501,8 +501,8 @@ void* tma_create(const GridView& G) {
 
 void tma_destroy(void* state) { delete (TmaMaps*)state; }
 
-static int choose_cz(const GridView& G) {
-  // one CTA per SM: pick the pencil length that minimises (waves of 148 CTAs) x (planes per CTA + the two
+static int choose_cz(const GridView& G, int sm_count) {
+  // one CTA per SM: pick the pencil length that minimises (waves of sm_count CTAs) x (planes per CTA + the two
   // lead-in z phases, ~2/3 of a plane)
   const long long tiles = (long long)((G.n[0] + TX - 1) / TX) * ((G.n[1] + TY - 1) / TY);
   int best = G.n[2];
@@ -511,15 +511,15 @@ static int choose_cz(const GridView& G) {
     const int cz = (G.n[2] + chunks - 1) / chunks;
     if (cz < 4 && chunks > 1) break;
     const long long ctas = tiles * ((G.n[2] + cz - 1) / cz);
-    const double cost = (double)((ctas + 147) / 148) * (cz + 0.7);
+    const double cost = (double)((ctas + sm_count - 1) / sm_count) * (cz + 0.7);
     if (cost < best_cost) { best_cost = cost; best = cz; }
   }
   return best;
 }
 
 template <int RECON, int CHARGE, int STAGE>
-static cudaError_t launch_one(const GridView& G, const TmaMaps& M, double dt, cudaStream_t st) {
-  const int cz = choose_cz(G);
+static cudaError_t launch_one(const GridView& G, const TmaMaps& M, double dt, int sm_count, cudaStream_t st) {
+  const int cz = choose_cz(G, sm_count);
   const PencilTabs T = make_tabs(G);
   dim3 block(NTHREADS, 1, 1);
   dim3 grid((G.n[0] + TX - 1) / TX, (G.n[1] + TY - 1) / TY, (G.n[2] + cz - 1) / cz);
@@ -531,24 +531,24 @@ static cudaError_t launch_one(const GridView& G, const TmaMaps& M, double dt, cu
 }
 
 template <int RECON, int CHARGE>
-static cudaError_t launch_rc(const GridView& G, const TmaMaps& M, double dt, int stage, cudaStream_t st) {
-  return stage == 1 ? launch_one<RECON, CHARGE, 1>(G, M, dt, st) : launch_one<RECON, CHARGE, 2>(G, M, dt, st);
+static cudaError_t launch_rc(const GridView& G, const TmaMaps& M, double dt, int stage, int sm_count, cudaStream_t st) {
+  return stage == 1 ? launch_one<RECON, CHARGE, 1>(G, M, dt, sm_count, st) : launch_one<RECON, CHARGE, 2>(G, M, dt, sm_count, st);
 }
 
-cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int stage, int recon, cudaStream_t st) {
+cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int stage, int recon, int sm_count, cudaStream_t st) {
   if (!state) return cudaErrorInvalidValue;
   const TmaMaps& M = *(const TmaMaps*)state;
   const bool ohm = G.charge_mode == CHARGE_FACE_OHM;
   switch (recon) {
     case RECON_MINMOD:
-      return ohm ? launch_rc<RECON_MINMOD, CHARGE_FACE_OHM>(G, M, dt, stage, st)
-                 : launch_rc<RECON_MINMOD, CHARGE_CELL_CURRENT>(G, M, dt, stage, st);
+      return ohm ? launch_rc<RECON_MINMOD, CHARGE_FACE_OHM>(G, M, dt, stage, sm_count, st)
+                 : launch_rc<RECON_MINMOD, CHARGE_CELL_CURRENT>(G, M, dt, stage, sm_count, st);
     case RECON_MC:
-      return ohm ? launch_rc<RECON_MC, CHARGE_FACE_OHM>(G, M, dt, stage, st)
-                 : launch_rc<RECON_MC, CHARGE_CELL_CURRENT>(G, M, dt, stage, st);
+      return ohm ? launch_rc<RECON_MC, CHARGE_FACE_OHM>(G, M, dt, stage, sm_count, st)
+                 : launch_rc<RECON_MC, CHARGE_CELL_CURRENT>(G, M, dt, stage, sm_count, st);
     default:
-      return ohm ? launch_rc<RECON_WENO5, CHARGE_FACE_OHM>(G, M, dt, stage, st)
-                 : launch_rc<RECON_WENO5, CHARGE_CELL_CURRENT>(G, M, dt, stage, st);
+      return ohm ? launch_rc<RECON_WENO5, CHARGE_FACE_OHM>(G, M, dt, stage, sm_count, st)
+                 : launch_rc<RECON_WENO5, CHARGE_CELL_CURRENT>(G, M, dt, stage, sm_count, st);
   }
 }
 

@@ -223,6 +223,60 @@ def test_device_pointers_and_stream(binding):
     assert g.launch_count() > 0
 
 
+def test_set_stream_orders_old_stream_work_before_new(binding):
+    """work enqueued on the old stream (here: the uploads and prim->cons of set_prims from device tensors,
+    kept busy behind a long copy) must be complete before a step enqueued on a NEW non-blocking stream reads the
+    state.  The library inserts an event/wait pair at the switch; without it the step reads a half-written state."""
+    import torch
+    w = wl.blast_curved()
+    n, bc = (48, 40, 24), (wl.BC_OUTFLOW,) * 3
+    f = w.fields((100, 108, 100), n)
+    ref_h = binding.from_workload(w, fields=f, n=n, bc=bc)
+    ref_h.step(w.dt, w.recon)
+    ref = ref_h.get_prims()
+    A, B = torch.cuda.Stream(), torch.cuda.Stream()          # both non-blocking with respect to the legacy stream
+    metric = torch.from_numpy(f["metric"]).cuda(); prims = torch.from_numpy(f["prims"]).cuda()
+    sigma = torch.from_numpy(f["sigma"]).cuda()
+    big = torch.zeros(1 << 27, dtype=torch.float64, device="cuda")      # 1 GiB: ~0.35 ms per device copy
+    big2 = torch.empty_like(big)
+    torch.cuda.synchronize()
+    for trial in range(3):
+        g = binding.Rgrmhd(w.params(n=n, bc=bc))
+        g.set_stream(A.cuda_stream)
+        with torch.cuda.stream(A):
+            for _ in range(8 * (trial + 1)):
+                big2.copy_(big)                                           # keep stream A busy ahead of the uploads
+        g.set_metric(metric); g.set_sigma(sigma); g.set_prims(prims)       # queued on A behind the copies
+        g.set_stream(B.cuda_stream)                                       # hand-over: B waits for A
+        g.step(w.dt, w.recon)
+        out = torch.empty_like(prims)
+        g.get_prims(out)
+        B.synchronize()
+        assert np.array_equal(out.cpu().numpy(), ref), trial
+        torch.cuda.synchronize()
+
+
+def test_failed_launch_poisons_handle_until_set_prims(binding):
+    """A launch that fails inside rgrmhd_step (here: a grid the recovery kernel cannot be launched on, n_y > 65535
+    rows) leaves the state half advanced: the step returns E_CUDA, every reader returns E_STATE until set_prims
+    replaces the state."""
+    n = (4, 65540, 1)
+    par = dict(n=n, dx=(0.1, 0.1, 0.1), bc=(1, 1, 1), gamma_eos=2.0, sigma0=1.0)
+    g = binding.Rgrmhd(par)
+    m = np.zeros((16,) + g.shape); m[0] = 1; m[4] = m[7] = m[9] = 1
+    P = np.zeros((14,) + g.shape); P[0] = 1; P[1] = 1
+    g.set_metric(m); g.set_prims(P)
+    with pytest.raises(binding.RgrmhdError) as e:
+        g.step(0.01, wl.RECON_MC)
+    assert e.value.code == -3
+    for call in (g.get_prims, g.get_cons, g.stats, g.flush, lambda: g.step(0.01, wl.RECON_MC)):
+        with pytest.raises(binding.RgrmhdError) as e:
+            call()
+        assert e.value.code == -2
+    g.set_prims(P)                                               # replaces the state: usable again
+    assert np.array_equal(interior(g.get_prims(), n), interior(P, n))
+
+
 def test_variants_agree_bitwise_or_to_roundoff(binding):
     """Tiled and simple RHS kernels evaluate the same expressions: agreement far inside the oracle
     tolerance on a block with a ragged tail in every direction."""
@@ -338,7 +392,7 @@ def _cut_slices(w, lo, shape, margin):
     for d in (2, 1, 0):                                        # arrays are (field, z, y, x)
         a = 0 if lo[d] == 0 else margin
         b = shape[d] if lo[d] + shape[d] == w.n[d] else shape[d] - margin
-        assert b - a >= 8, "sub-block too small for its margin"
+        assert b - a >= 4, "sub-block too small for its margin"
         sl_o.append(slice(a, b))
         sl_g.append(slice(3 + lo[d] + a, 3 + lo[d] + b))
     return tuple(sl_o), tuple(sl_g)
@@ -469,14 +523,14 @@ def cfg2_oracle_run():
 
 def test_cfg2_current_sheet_all_9600_steps(binding, cfg2_oracle_run):
     """BASELINE config 2 in full: 800 cells, 9600 steps to t = 10, against the oracle (one core: a 1D block has too
-    little work per step for threads).  Smooth diffusion, no limiter switches; round-off differences accumulate at
-    most linearly, so the bound is the 20-step one scaled by 9600/20 (as config 1's full run scales it)."""
+    little work per step for threads).  Smooth diffusion, no limiter switches: the 20-step bound 1e-9 holds for the
+    whole run (measured 4.8e-12)."""
     w, f, bg = cfg2_oracle_run
     g = binding.from_workload(w, fields=f)
     for _ in range(w.nsteps):
         g.step(w.dt, w.recon)
     o = bg.result()
-    worst = _compare(g, o, w.n, w.dx[0], (w.nsteps / 20) * TOL20, "cfg2 t=10")
+    worst = _compare(g, o, w.n, w.dx[0], TOL20, "cfg2 t=10")
     assert g.stats()["c2p_failures"] == 0 and o.stats()["c2p_failures"] == 0
     print("cfg2 800 x 9600 steps: worst rel Linf %.2e" % worst)
 
