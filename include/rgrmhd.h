@@ -62,9 +62,18 @@ enum { RGRMHD_SIGMA_UNIFORM = 0, RGRMHD_SIGMA_ARRAY = 1, RGRMHD_SIGMA_POWER_D = 
  *   FACE_OHM     Ohm's law (Eq. 29) on the reconstructed left/right states, sigma_L/R = cell sigma
  *   CELL_CURRENT (default) the cell-centred conduction current fixed by the implicit solve of the
  *                same stage, J_c = (calE* - calE)/(a_ii dt alpha), reconstructed like a primitive
- *   DIV_E        not evolved: q = div E after each stage -- NOT BUILT YET: create
- *                returns RGRMHD_E_INVALID. */
+ *   DIV_E        the charge is not evolved: q = nabla_i E^i of each stage's electric field,
+ *                second-order centred differences of sqrt(gamma) E^i (reading R15); the
+ *                new state's q and calQ are computed when the state is read. */
 enum { RGRMHD_CHARGE_FACE_OHM = 0, RGRMHD_CHARGE_CELL_CURRENT = 1, RGRMHD_CHARGE_DIV_E = 2 };
+
+/* characteristic speeds of HLLE and of the CFL reduction:
+ *   LIGHT       lambda+- = +-alpha sqrt(gamma^kk) - beta^k everywhere (Eq. 30; default)
+ *   MHD_INSIDE  the paper's alternative: the ideal-GRMHD value inside the star, the speed
+ *               of light outside.  Ideal-GRMHD value = the fast-magnetosonic bound a^2 = cs^2 + vA^2 - cs^2 vA^2
+ *               boosted to the coordinate frame (reading R16), envelope of the two face states;
+ *               "inside" = both face states have rho > wave_rho_switch. */
+enum { RGRMHD_WAVE_LIGHT = 0, RGRMHD_WAVE_MHD_INSIDE = 1 };
 
 /* `scheme` argument of rgrmhd_step = reconstruction | time scheme */
 enum { RGRMHD_RECON_MINMOD = 0, RGRMHD_RECON_MC = 1, RGRMHD_RECON_WENO5 = 2, RGRMHD_RECON_MASK = 0xff };
@@ -86,6 +95,8 @@ typedef struct {
   int    charge_mode; /* RGRMHD_CHARGE_*                                                          */
   double weno_eps;    /* WENO5 regulariser; <= 0 selects 1e-26 (reading R5)             */
   int    device;      /* CUDA device ordinal                                                      */
+  int    wave_speed_mode;  /* RGRMHD_WAVE_*: characteristic speeds of the HLLE solver                     */
+  double wave_rho_switch;  /* MHD_INSIDE: "inside the star" = both face states denser than this           */
 } rgrmhd_params;
 
 typedef struct {
@@ -137,7 +148,8 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme);
 int rgrmhd_flush(rgrmhd_t h);
 
 /* max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k
- * (Eq. 30); dt = CFL / that.  Synchronises. */
+ * (Eq. 30); dt = CFL / that.  With wave_speed_mode MHD_INSIDE a cell with rho > wave_rho_switch contributes
+ * max(|lambda-|, |lambda+|)/dx^k of its own state instead (needs set_prims; a per-step reduction).  Synchronises. */
 int rgrmhd_max_speed(rgrmhd_t h, double* host_out);
 
 /* Current primitives (ghost zones filled by the boundary rule) / conserved variables

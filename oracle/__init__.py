@@ -45,7 +45,7 @@ class Params(C.Structure):
                 ("sigma_exp", C.c_double), ("sigma_dref", C.c_double), ("kappa", C.c_double),
                 ("rho_floor", C.c_double), ("k_atmo", C.c_double), ("c2p_tol", C.c_double),
                 ("c2p_max_iter", C.c_int), ("charge_mode", C.c_int), ("weno_eps", C.c_double),
-                ("device", C.c_int)]
+                ("device", C.c_int), ("wave_speed_mode", C.c_int), ("wave_rho_switch", C.c_double)]
 
 
 class Stats(C.Structure):
@@ -98,6 +98,7 @@ def make_params(p: dict) -> Params:
     q.rho_floor = p.get("rho_floor", 0.0); q.k_atmo = p.get("k_atmo", 0.0); q.c2p_tol = p.get("c2p_tol", 0.0)
     q.c2p_max_iter = int(p.get("c2p_max_iter", 0)); q.charge_mode = int(p.get("charge_mode", 1))
     q.weno_eps = p.get("weno_eps", 0.0); q.device = 0
+    q.wave_speed_mode = int(p.get("wave_speed_mode", 0)); q.wave_rho_switch = p.get("wave_rho_switch", 0.0)
     return q
 
 
@@ -229,6 +230,15 @@ def prim2cons_point(P, gamma_eos, alpha=1.0, beta=None, g6=None):
     lib().oracle_prim2cons_point(C.c_double(gamma_eos), C.c_double(alpha), _dp(_a(beta, 3)) if beta is not None else None,
                                  _dp(_a(_G_FLAT if g6 is None else g6, 6)), _dp(_a(P, 14)), _dp(U))
     return U
+
+
+def wave_speeds_point(P, k, gamma_eos, alpha=1.0, beta=None, g6=None):
+    """(lambda-, lambda+) of the ideal-GRMHD bound (A9) for one state in direction k."""
+    lm, lp = C.c_double(), C.c_double()
+    lib().oracle_wave_speeds_point(C.c_double(gamma_eos), C.c_double(alpha), _dp(_a(beta, 3)) if beta is not None else None,
+                                   _dp(_a(_G_FLAT if g6 is None else g6, 6)), C.c_int(k), _dp(_a(P, 14)),
+                                   C.byref(lm), C.byref(lp))
+    return lm.value, lp.value
 
 
 def sigma_point(model, sigma0, sigma_exp, sigma_dref, Dhat, sigma_cell=0.0):

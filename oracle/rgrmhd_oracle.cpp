@@ -48,6 +48,7 @@ enum { BC_PERIODIC = 0, BC_OUTFLOW = 1 };
 enum { SIGMA_UNIFORM = 0, SIGMA_ARRAY = 1, SIGMA_POWER_D = 2, SIGMA_ATMO = 3 };
 enum { CHARGE_FACE_OHM = 0, CHARGE_CELL_CURRENT = 1, CHARGE_DIV_E = 2 };
 enum { RECON_MINMOD = 0, RECON_MC = 1, RECON_WENO5 = 2 };
+enum { WAVE_LIGHT = 0, WAVE_MHD_INSIDE = 1 };
 
 // permutation symbol [ijk]
 inline double perm(int i, int j, int k) { return 0.5 * (i - j) * (j - k) * (k - i); }
@@ -136,6 +137,7 @@ void prim2cons_point(const Metric& m, double Gamma, const double P[NPRIM], doubl
 //   F(calQ)=alpha J^k - beta^k calQ, J^k = calQ v^k + Jc^k  (Eq. 29)
 //   Jc^k: charge_mode FACE_OHM : W sigma [calE^k + sqrt(g)(v x B)^k - (v.E) sqrt(g) v^k]
 //         charge_mode CELL_CURRENT : sqrt(g) * jck, jck = reconstructed undensitised cell current
+//         charge_mode DIV_E : as CELL_CURRENT; the evolved calQ is discarded (charge_from_div_E replaces it)
 // ---------------------------------------------------------------------------------------------
 void state_flux(const Metric& m, double Gamma, int k, const double P[NPRIM], int charge_mode,
                 double sigma, double jck, double U[NCONS], double F[NCONS]) {
@@ -227,6 +229,7 @@ struct Params {
   int n[3]; double dx[3]; int ng; int bc[3];
   double Gamma; int sigma_model; double sigma0, sigma_exp, sigma_dref;
   double kappa, rho_floor, k_atmo, c2p_tol; int c2p_max_iter; int charge_mode; double weno_eps;
+  int wave_speed_mode; double wave_rho_switch;
 };
 
 double sigma_of(const Params& p, double Dhat, double sigma_cell) {
@@ -640,6 +643,32 @@ void metric_face(const Grid& G, long cL, long cR, Metric& m) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// A9. characteristic speeds "used in ideal GRMHD" (reading R16).  The ideal-GRMHD HLLE solvers
+// bound the fast magnetosonic speed in the fluid frame by
+//   a^2 = cs^2 + vA^2 - cs^2 vA^2,   cs^2 = Gamma p / h (Eq. 50 in reading G3),   vA^2 = b^2/(h + b^2),
+//   b^2 = B^2/W^2 + (B.v)^2  (comoving field of ideal MHD; h = enthalpy density)
+// and boost it to the Eulerian coordinate frame along direction k:
+//   lambda+- = alpha [ v^k (1 - a^2) +- sqrt( a^2 (1 - v^2) [ gamma^kk (1 - v^2 a^2) - v^k v^k (1 - a^2) ] ) ] / (1 - v^2 a^2) - beta^k.
+// With a = 1 this is Eq. 30's light cone, +-alpha sqrt(gamma^kk) - beta^k.
+// ---------------------------------------------------------------------------------------------
+void mhd_wave_speeds(const Metric& m, double Gamma, int k, const double P[NPRIM], double* lam_minus, double* lam_plus) {
+  const double rho = P[RHO], p = P[PRS];
+  const double vU[3] = {P[VX], P[VY], P[VZ]}, BU[3] = {P[BX], P[BY], P[BZ]};
+  double vD[3], BD[3];
+  lower(m, vU, vD); lower(m, BU, BD);
+  const double v2 = dotUD(vU, vD), B2 = dotUD(BU, BD), Bv = dotUD(BU, vD);
+  const double h = rho * (1.0 + p / ((Gamma - 1.0) * rho)) + p;
+  const double b2 = B2 * (1.0 - v2) + Bv * Bv;
+  const double cs2 = Gamma * p / h, vA2 = b2 / (h + b2);
+  const double a2 = cs2 + vA2 - cs2 * vA2;
+  const double den = 1.0 - v2 * a2;
+  const double disc = a2 * (1.0 - v2) * (m.gUU[k][k] * den - vU[k] * vU[k] * (1.0 - a2));
+  const double root = std::sqrt(std::max(disc, 0.0));
+  *lam_plus = m.alpha * (vU[k] * (1.0 - a2) + root) / den - m.betaU[k];
+  *lam_minus = m.alpha * (vU[k] * (1.0 - a2) - root) / den - m.betaU[k];
+}
+
+// ---------------------------------------------------------------------------------------------
 // a1. ghost fill ("copied from the nearest interior point"; PAPER.md:359 periodic);
 //     x, then y, then z, each over the full padded extent of the other directions (reading R10).
 // ---------------------------------------------------------------------------------------------
@@ -731,9 +760,20 @@ int hlle_face(const Grid& G, int scheme, int d, int i, int j, int k, double Fh[N
   double UL[NCONS], FL[NCONS], UR[NCONS], FR[NCONS];
   state_flux(mf, G.par.Gamma, d, PL, G.par.charge_mode, sigL, jL, UL, FL);
   state_flux(mf, G.par.Gamma, d, PR, G.par.charge_mode, sigR, jR, UR, FR);
-  const double c = mf.alpha * std::sqrt(mf.gUU[d][d]);
-  const double lp = std::max(0.0, c - mf.betaU[d]);
-  const double lm = std::min(0.0, -c - mf.betaU[d]);
+  double lp, lm;
+  if (G.par.wave_speed_mode == WAVE_MHD_INSIDE && PL[RHO] > G.par.wave_rho_switch && PR[RHO] > G.par.wave_rho_switch) {
+    // reading R16: "inside the star" = both face states denser than wave_rho_switch; the ideal-GRMHD bound of
+    // both states, HLLE's usual envelope
+    double lmL, lpL, lmR, lpR;
+    mhd_wave_speeds(mf, G.par.Gamma, d, PL, &lmL, &lpL);
+    mhd_wave_speeds(mf, G.par.Gamma, d, PR, &lmR, &lpR);
+    lp = std::max(0.0, std::max(lpL, lpR));
+    lm = std::min(0.0, std::min(lmL, lmR));
+  } else {
+    const double c = mf.alpha * std::sqrt(mf.gUU[d][d]);
+    lp = std::max(0.0, c - mf.betaU[d]);
+    lm = std::min(0.0, -c - mf.betaU[d]);
+  }
   for (int v = 0; v < NCONS; ++v) Fh[v] = (lp * FL[v] - lm * FR[v] + lp * lm * (UR[v] - UL[v])) / (lp - lm);
   return fixups;
 }
@@ -902,19 +942,58 @@ void solve_all(Grid& G, std::vector<double> Ust[NCONS], double adt, std::vector<
 }
 
 // ---------------------------------------------------------------------------------------------
+// A22. charge_mode DIV_E: the charge density is not evolved but computed from the electric
+// field of the stage, q = nabla_i E^i = d_i(sqrt(gamma) E^i)/sqrt(gamma).  Reading R15 (the paper names no
+// stencil): second-order centred differences of calE^i = sqrt(gamma) E^i, inactive directions dropped.  Needs
+// the ghost zones of E^i filled.  Writes q into P (interior) and, if asked, calQ = sqrt(gamma) q into Un.
+// ---------------------------------------------------------------------------------------------
+void charge_from_div_E(Grid& G, bool write_cons) {
+  const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2];
+  const long stride[3] = {1, (long)G.np[0], (long)G.np[0] * G.np[1]};
+#pragma omp parallel for collapse(3) schedule(static)
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const long c = G.idx(i, j, k);
+        Metric m; metric_at(G, c, m);
+        double div = 0.0;
+        for (int d = 0; d < 3; ++d) {
+          if (!G.active(d)) continue;
+          Metric mp, mm; metric_at(G, c + stride[d], mp); metric_at(G, c - stride[d], mm);
+          div += (mp.sqrtg * G.P[EX + d][c + stride[d]] - mm.sqrtg * G.P[EX + d][c - stride[d]]) / (2.0 * G.par.dx[d]);
+        }
+        G.P[QCH][c] = div / m.sqrtg;
+        if (write_cons) G.Un[CQ][c] = div;
+      }
+}
+
+// ---------------------------------------------------------------------------------------------
 // O2. one IMEX-SSP2(2,2,2) step (Eq. 35-37; gamma = 1 - 1/sqrt(2)).
 //   Table I's body is missing from the text; Eq. 35-37 fix it: explicit A~=[[0,0],[1,0]], w~=(1/2,1/2);
 //   implicit A=[[g,0],[1-2g,g]], w=(1/2,1/2).   X = calE^i (stiff), Y = the other 11.
 //   R[U^(i)] is evaluated as the difference quotient (X^(i) - X*^(i))/(g dt) (reading R11).
 // ---------------------------------------------------------------------------------------------
+// after a stage's solve: ghost zones of the stage primitives and of the conduction current; in charge mode DIV_E
+// the stage's charge density from its electric field (A22), ghost-filled in turn
+void stage_ghosts_and_charge(Grid& G) {
+  for (int v = 0; v < NPRIM; ++v) ghost_fill_field(G, G.P[v]);
+  for (int q = 0; q < 3; ++q) ghost_fill_field(G, G.jc[q]);
+  if (G.par.charge_mode == CHARGE_DIV_E) { charge_from_div_E(G, false); ghost_fill_field(G, G.P[QCH]); }
+}
+// charge mode DIV_E: the new state's q and calQ from its electric field
+void final_charge(Grid& G) {
+  if (G.par.charge_mode != CHARGE_DIV_E) return;
+  for (int q = 0; q < 3; ++q) ghost_fill_field(G, G.P[EX + q]);
+  charge_from_div_E(G, true);
+}
+
 void step(Grid& G, double dt, int scheme) {
   const double gam = 1.0 - 1.0 / std::sqrt(2.0);
   const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2];
   // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n
   solve_all(G, G.Un, gam * dt, G.X1, false);
   for (int q = 0; q < 3; ++q) G.jc1[q] = G.jc[q];
-  for (int v = 0; v < NPRIM; ++v) ghost_fill_field(G, G.P[v]);
-  for (int q = 0; q < 3; ++q) ghost_fill_field(G, G.jc[q]);
+  stage_ghosts_and_charge(G);
   rhs_all(G, scheme, G.F1);
   // stage 2 (Eq. 36)
 #pragma omp parallel for collapse(3) schedule(static)
@@ -928,8 +1007,7 @@ void step(Grid& G, double dt, int scheme) {
     }
   }
   solve_all(G, G.Us, gam * dt, G.X2, false);
-  for (int v = 0; v < NPRIM; ++v) ghost_fill_field(G, G.P[v]);
-  for (int q = 0; q < 3; ++q) ghost_fill_field(G, G.jc[q]);
+  stage_ghosts_and_charge(G);
   rhs_all(G, scheme, G.F2);
   // final combination (Eq. 37)
 #pragma omp parallel for collapse(3) schedule(static)
@@ -946,15 +1024,28 @@ void step(Grid& G, double dt, int scheme) {
   }
   // recovery of the new state at fixed calE (reading R12), guess = P^(2)
   solve_all(G, G.Un, 0.0, nullptr, true);
+  final_charge(G);
 }
 
-// a7. max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k (Eq. 30)
+// a7. max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k (Eq. 30); with
+// wave_speed_mode MHD_INSIDE (A9) the cell's own max(|lambda-|, |lambda+|)/dx^k where rho > wave_rho_switch
 double max_speed(const Grid& G) {
   double mx = 0.0;
   for (int k = 0; k < G.par.n[2]; ++k) for (int j = 0; j < G.par.n[1]; ++j) for (int i = 0; i < G.par.n[0]; ++i) {
-    Metric m; metric_at(G, G.idx(i, j, k), m);
-    for (int d = 0; d < 3; ++d) if (G.active(d))
-      mx = std::max(mx, (m.alpha * std::sqrt(m.gUU[d][d]) + std::fabs(m.betaU[d])) / G.par.dx[d]);
+    const long c = G.idx(i, j, k);
+    Metric m; metric_at(G, c, m);
+    const bool mhd = G.par.wave_speed_mode == WAVE_MHD_INSIDE && G.have_prims && G.P[RHO][c] > G.par.wave_rho_switch;
+    double P[NPRIM];
+    if (mhd) for (int v = 0; v < NPRIM; ++v) P[v] = G.P[v][c];
+    for (int d = 0; d < 3; ++d) if (G.active(d)) {
+      if (mhd) {       // A9: the cell's own ideal-GRMHD speeds where it counts as "inside the star"
+        double lm, lp;
+        mhd_wave_speeds(m, G.par.Gamma, d, P, &lm, &lp);
+        mx = std::max(mx, std::max(std::fabs(lm), std::fabs(lp)) / G.par.dx[d]);
+      } else {
+        mx = std::max(mx, (m.alpha * std::sqrt(m.gUU[d][d]) + std::fabs(m.betaU[d])) / G.par.dx[d]);
+      }
+    }
   }
   return mx;
 }
@@ -992,6 +1083,7 @@ struct oracle_params {
   int n[3]; double dx[3]; int ng; int bc[3]; double gamma_eos; int sigma_model;
   double sigma0, sigma_exp, sigma_dref, kappa, rho_floor, k_atmo, c2p_tol; int c2p_max_iter;
   int charge_mode; double weno_eps; int device;
+  int wave_speed_mode; double wave_rho_switch;
 };
 struct oracle_stats { long long c2p_solves, c2p_evals, c2p_failures, floor_resets; int c2p_max_evals, reserved; };
 
@@ -999,7 +1091,8 @@ int oracle_create(void** out, const oracle_params* p) {
   if (!out || !p) return -1;
   if (p->ng != 3 || !(p->gamma_eos > 1.0)) return -1;
   for (int d = 0; d < 3; ++d) if (p->n[d] < 1 || (p->n[d] > 1 && !(p->dx[d] > 0.0)) || p->bc[d] < 0 || p->bc[d] > 1) return -1;
-  if (p->sigma_model < 0 || p->sigma_model > 3 || p->charge_mode < 0 || p->charge_mode > 1) return -1;
+  if (p->sigma_model < 0 || p->sigma_model > 3 || p->charge_mode < 0 || p->charge_mode > 2) return -1;
+  if (p->wave_speed_mode < 0 || p->wave_speed_mode > 1) return -1;
   Grid* G = new Grid();
   Params& q = G->par;
   for (int d = 0; d < 3; ++d) { q.n[d] = p->n[d]; q.dx[d] = p->dx[d]; q.bc[d] = p->bc[d]; }
@@ -1008,6 +1101,7 @@ int oracle_create(void** out, const oracle_params* p) {
   q.c2p_tol = p->c2p_tol > 0 ? p->c2p_tol : 8.0 * std::ldexp(1.0, -52);
   q.c2p_max_iter = p->c2p_max_iter > 0 ? p->c2p_max_iter : 100;
   q.charge_mode = p->charge_mode; q.weno_eps = p->weno_eps > 0 ? p->weno_eps : 1e-26;
+  q.wave_speed_mode = p->wave_speed_mode; q.wave_rho_switch = p->wave_rho_switch;
   G->ntot = 1;
   for (int d = 0; d < 3; ++d) { G->g[d] = q.n[d] > 1 ? 3 : 0; G->np[d] = q.n[d] + 2 * G->g[d]; G->ntot *= G->np[d]; }
   for (int v = 0; v < NMET; ++v) G->met[v].assign(G->ntot, 0.0);
@@ -1160,6 +1254,13 @@ int oracle_c2p_plain_point(double Gamma, double alpha, const double* g6, const d
   C2PResult r = c2p_plain(m, Gamma, U, adt, sigma, tol > 0 ? tol : 8.0 * std::ldexp(1.0, -52),
                           max_outer > 0 ? max_outer : PLAIN_MAX_OUTER, P);
   return r.failed ? -(r.evals + 1) : r.evals;
+}
+// A9: lambda-, lambda+ of one state at one point in direction k
+int oracle_wave_speeds_point(double Gamma, double alpha, const double* beta3, const double* g6, int k, const double* P,
+                             double* lam_minus, double* lam_plus) {
+  Metric m = metric_from_arrays(alpha, beta3, g6);
+  mhd_wave_speeds(m, Gamma, k, P, lam_minus, lam_plus);
+  return 0;
 }
 // conductivity models at one point (A18)
 double oracle_sigma_point(int model, double sigma0, double sigma_exp, double sigma_dref, double Dhat, double sigma_cell) {

@@ -35,7 +35,7 @@ class Params(C.Structure):
                 ("sigma_exp", C.c_double), ("sigma_dref", C.c_double), ("kappa", C.c_double),
                 ("rho_floor", C.c_double), ("k_atmo", C.c_double), ("c2p_tol", C.c_double),
                 ("c2p_max_iter", C.c_int), ("charge_mode", C.c_int), ("weno_eps", C.c_double),
-                ("device", C.c_int)]
+                ("device", C.c_int), ("wave_speed_mode", C.c_int), ("wave_rho_switch", C.c_double)]
 
 
 class Stats(C.Structure):
@@ -107,10 +107,10 @@ def make_params(p: dict, device: int = 0) -> Params:
     q = params_default()
     q.n[:] = list(p["n"]); q.dx[:] = list(p["dx"]); q.ng = int(p.get("ng", 3)); q.bc[:] = list(p["bc"])
     q.gamma_eos = p["gamma_eos"]
-    for k in ("sigma_model", "c2p_max_iter", "charge_mode"):
+    for k in ("sigma_model", "c2p_max_iter", "charge_mode", "wave_speed_mode"):
         if k in p:
             setattr(q, k, int(p[k]))
-    for k in ("sigma0", "sigma_exp", "sigma_dref", "kappa", "rho_floor", "k_atmo", "c2p_tol", "weno_eps"):
+    for k in ("sigma0", "sigma_exp", "sigma_dref", "kappa", "rho_floor", "k_atmo", "c2p_tol", "weno_eps", "wave_rho_switch"):
         if k in p:
             setattr(q, k, float(p[k]))
     q.device = int(device)

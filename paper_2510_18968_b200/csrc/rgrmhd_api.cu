@@ -23,7 +23,8 @@ cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int 
 void* tma_create(const GridView& G);
 void tma_destroy(void* state);
 cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, cudaStream_t st);
-cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, int sm_count, cudaStream_t st);
+cudaError_t launch_charge_div_e(const GridView& G, int stage, double dt, cudaStream_t st);
+cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, bool have_prims, int sm_count, cudaStream_t st);
 }  // namespace rg
 
 struct rgrmhd_s {
@@ -41,6 +42,7 @@ struct rgrmhd_s {
   bool pending_final = false;   // the last step's final recovery (k_c2p<3>) has not been launched yet
   bool poisoned = false;        // a launch inside rgrmhd_step failed: the state is half advanced until set_prims replaces it
   int sm_count = 148;           // multiprocessors of the device (grid sizing of the flux and reduction kernels)
+  bool charge_final_due = false;   // charge mode DIV_E: q, calQ of the new state not computed yet (done on output)
   int last_rhs_variant = -1;    // flux kernel the last rgrmhd_step actually launched
   int rhs_variant = 0;               // 0 = TMA-staged (default), 1 = simple, 2 = pencil (global-memory stencils)
   void* tma = nullptr;               // tensor maps of the TMA-staged flux kernel (null: shape not supported)
@@ -105,11 +107,13 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
     if (p->bc[d] != RGRMHD_BC_PERIODIC && p->bc[d] != RGRMHD_BC_OUTFLOW) return RGRMHD_E_INVALID;
   }
   if (p->sigma_model < RGRMHD_SIGMA_UNIFORM || p->sigma_model > RGRMHD_SIGMA_ATMO) return RGRMHD_E_INVALID;
-  if (p->charge_mode != RGRMHD_CHARGE_FACE_OHM && p->charge_mode != RGRMHD_CHARGE_CELL_CURRENT)
-    return RGRMHD_E_INVALID;                                     // DIV_E: not built
+  if (p->charge_mode != RGRMHD_CHARGE_FACE_OHM && p->charge_mode != RGRMHD_CHARGE_CELL_CURRENT &&
+      p->charge_mode != RGRMHD_CHARGE_DIV_E)
+    return RGRMHD_E_INVALID;
   if (p->sigma_model == RGRMHD_SIGMA_POWER_D &&
       (p->sigma_exp < 0.0 || std::fabs(p->sigma_exp - std::lround(p->sigma_exp)) > 0.0 || !(p->sigma_dref > 0.0)))
     return RGRMHD_E_INVALID;
+  if (p->wave_speed_mode != RGRMHD_WAVE_LIGHT && p->wave_speed_mode != RGRMHD_WAVE_MHD_INSIDE) return RGRMHD_E_INVALID;
   if (p->weno_eps > 0.0 && p->weno_eps < 1e-60) return RGRMHD_E_INVALID;   // product-form weights would underflow
   if (p->rho_floor < 0.0 || !(p->kappa == p->kappa)) return RGRMHD_E_INVALID;
 
@@ -150,6 +154,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   G.tol = p->c2p_tol > 0.0 ? p->c2p_tol : 8.0 * std::ldexp(1.0, -52);
   G.maxit = p->c2p_max_iter > 0 ? p->c2p_max_iter : 100;
   G.charge_mode = p->charge_mode;
+  G.wave_mode = p->wave_speed_mode; G.wave_rho_switch = p->wave_rho_switch;
   G.weno_eps = p->weno_eps > 0.0 ? p->weno_eps : 1e-26;
 
   const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3 + rg::NSRC + rg::NCONS;
@@ -229,6 +234,20 @@ static int finish_step(rgrmhd_t h) {
   if (e != cudaSuccess) { h->poisoned = true; return fail_cuda(h, e, "launch_c2p(final recovery)"); }
   ++h->launches;
   h->pending_final = false;
+  return RGRMHD_OK;
+}
+
+// charge mode DIV_E: q and calQ of the new state from its electric field, when somebody reads the state
+static int finish_charge(rgrmhd_t h) {
+  if (!h->charge_final_due) return RGRMHD_OK;
+  const rg::GridView& G = h->G;
+  if (G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1) {
+    RG_CUDA(h, rg::launch_ghost_fill(G, G.P + rg::EX, 3, h->stream));
+    ++h->launches;
+  }
+  RG_CUDA(h, rg::launch_charge_div_e(G, 3, 0.0, h->stream));
+  ++h->launches;
+  h->charge_final_due = false;
   return RGRMHD_OK;
 }
 
@@ -325,6 +344,7 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]) {
   RG_CUDA(h, rg::launch_prim2cons(h->G, h->stream));
   ++h->launches;
   h->have_prims = true;
+  h->charge_final_due = false;
   return RGRMHD_OK;
 }
 
@@ -341,7 +361,8 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   double* ghost_fields[rg::NPRIM + 3];
   for (int v = 0; v < rg::NPRIM; ++v) ghost_fields[v] = G.P[v];
   for (int q = 0; q < 3; ++q) ghost_fields[rg::NPRIM + q] = G.jc[q];
-  const int nghost_fields = rg::NPRIM + (G.charge_mode == rg::CHARGE_CELL_CURRENT ? 3 : 0);
+  const int nghost_fields = rg::NPRIM + (G.charge_mode != rg::CHARGE_FACE_OHM ? 3 : 0);
+  const bool div_e = G.charge_mode == rg::CHARGE_DIV_E;
   const bool any_active = G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1;
   const bool tma = h->rhs_variant == 0 && h->tma != nullptr;
   const bool pencil = !tma && h->rhs_variant != 1 && rg::rhs_pencil_supported(G);
@@ -365,16 +386,19 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, first, dt, h->stats_dev, st); }));
   h->pending_final = false;
   if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  if (div_e) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_div_e(G, 1, dt, st); }));
   RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
   // stage 2 (Eq. 36)
   RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
   if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+  if (div_e) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_div_e(G, 2, dt, st); }));
   RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
 #undef RG_STEP
   // recovery of the new state at fixed calE (reading R12): deferred, see finish_step
   h->pending_final = true;
+  h->charge_final_due = div_e;
   h->solves += 3 * nint;
-  h->launches += 4 + (any_active ? 2 : 0);
+  h->launches += 4 + (any_active ? 2 : 0) + (div_e ? 2 : 0);
   return RGRMHD_OK;
 }
 
@@ -383,7 +407,11 @@ int rgrmhd_max_speed(rgrmhd_t h, double* host_out) {
   if (!h->have_metric) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   RG_CUDA(h, cudaMemsetAsync(h->maxspeed_dev, 0, sizeof(unsigned long long), h->stream));
-  RG_CUDA(h, rg::launch_max_speed(h->G, h->maxspeed_dev, h->sm_count, h->stream));
+  if (h->G.wave_mode == rg::WAVE_MHD_INSIDE && h->have_prims) {   // state dependent: needs the current primitives
+    int rc;
+    if ((rc = finish_step(h))) return rc;
+  }
+  RG_CUDA(h, rg::launch_max_speed(h->G, h->maxspeed_dev, h->have_prims, h->sm_count, h->stream));
   ++h->launches;
   unsigned long long bits = 0;
   RG_CUDA(h, cudaMemcpyAsync(&bits, h->maxspeed_dev, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
@@ -401,6 +429,7 @@ int rgrmhd_get_prims(rgrmhd_t h, double* const prims[14]) {
   DeviceGuard guard(h->device);
   int rc;
   if ((rc = finish_step(h))) return rc;
+  if ((rc = finish_charge(h))) return rc;
   const rg::GridView& G = h->G;
   if (G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1) {
     RG_CUDA(h, rg::launch_ghost_fill(G, G.P, rg::NPRIM, h->stream));
@@ -417,6 +446,7 @@ int rgrmhd_get_cons(rgrmhd_t h, double* const cons[14]) {
   DeviceGuard guard(h->device);
   int rc;
   if ((rc = finish_step(h))) return rc;
+  if ((rc = finish_charge(h))) return rc;
   for (int v = 0; v < rg::NCONS; ++v) if ((rc = copy_out(h, cons[v], h->G.Un[v]))) return rc;
   return RGRMHD_OK;
 }

@@ -22,8 +22,9 @@ enum { CD = 0, CSX, CSY, CSZ, CTAU, CEX, CEY, CEZ, CBX, CBY, CBZ, CPSI, CPHI, CQ
 enum { MALP = 0, MBX, MBY, MBZ, MGXX, MGXY, MGXZ, MGYY, MGYZ, MGZZ, MKXX, MKXY, MKXZ, MKYY, MKYZ, MKZZ };
 enum { BC_PERIODIC = 0, BC_OUTFLOW = 1 };
 enum { SIGMA_UNIFORM = 0, SIGMA_ARRAY = 1, SIGMA_POWER_D = 2, SIGMA_ATMO = 3 };
-enum { CHARGE_FACE_OHM = 0, CHARGE_CELL_CURRENT = 1 };
+enum { CHARGE_FACE_OHM = 0, CHARGE_CELL_CURRENT = 1, CHARGE_DIV_E = 2 };
 enum { RECON_MINMOD = 0, RECON_MC = 1, RECON_WENO5 = 2 };
+enum { WAVE_LIGHT = 0, WAVE_MHD_INSIDE = 1 };
 
 // Device view of one block: geometry, model constants and the SoA field pointers (all DEVICE memory,
 // padded layout of include/rgrmhd.h).  Passed to kernels by value as a __grid_constant__ parameter.
@@ -38,6 +39,8 @@ struct GridView {
   double Gamma, sigma0, sigma_dref, kappa, rho_floor, p_atmo, tol, weno_eps;
   double gog1, gm1og;    // Gamma/(Gamma-1), (Gamma-1)/Gamma (host-computed: no division in the kernels)
   int sigma_model, sigma_exp, maxit, charge_mode;
+  int wave_mode;             // WAVE_LIGHT | WAVE_MHD_INSIDE (reading R16)
+  double wave_rho_switch;    // MHD_INSIDE: both face states (or the cell) denser than this count as inside the star
   const double* met[NMET];
   const double* sigma;   // SIGMA_ARRAY only, else nullptr
   double* P[NPRIM];      // primitives of the current stage (ghosts filled by k_ghost_fill)
@@ -452,23 +455,60 @@ __device__ __forceinline__ void limit_velocity(const Met& m, double P[NPRIM]) {
   }
 }
 
-// a3 (second half). HLLE combination (Eq. 30; reading R6)
+// A9. characteristic speeds "used in ideal GRMHD" (reading R16) of one state along direction K:
+// the fluid-frame bound of the fast speed a^2 = cs^2 + vA^2 - cs^2 vA^2 (cs^2 = Gamma p/h, vA^2 = b^2/(h + b^2),
+// b^2 = B^2/W^2 + (B.v)^2) boosted to the coordinate frame,
+//   lambda+- = alpha [v^K (1-a^2) +- sqrt(a^2 (1-v^2) [gamma^KK (1 - v^2 a^2) - v^K v^K (1-a^2)])]/(1 - v^2 a^2) - beta^K.
+// Arguments: the scalars v^2, B^2, B.v (taken with the face/cell metric), v^K, gamma^KK.
+__device__ __forceinline__ void mhd_speeds(double alpha, double betaK, double giKK, double Gamma, double gog1, double rho,
+                                           double p, double v2, double B2, double Bv, double vK, double& lm, double& lp) {
+  const double h = rho + gog1 * p;
+  const double b2 = B2 * (1.0 - v2) + Bv * Bv;
+  const double cs2 = Gamma * p / h, vA2 = b2 / (h + b2);
+  const double a2 = cs2 + vA2 - cs2 * vA2;
+  const double den = 1.0 - v2 * a2, om = 1.0 - a2;
+  const double root = sqrt(fmax(a2 * (1.0 - v2) * (giKK * den - vK * vK * om), 0.0));
+  const double iden = 1.0 / den;
+  lp = alpha * (vK * om + root) * iden - betaK;
+  lm = alpha * (vK * om - root) * iden - betaK;
+}
+// natural-frame wrapper: P = primitives (after the fix-ups of reading R4), m = face or cell metric
+template <int K>
+__device__ __forceinline__ void mhd_speeds_nat(const Met& m, double Gamma, const double P[NPRIM], double& lm, double& lp) {
+  const double vU[3] = {P[VX], P[VY], P[VZ]}, BU[3] = {P[BX], P[BY], P[BZ]};
+  double vD[3], BD[3];
+  lower(m, vU, vD); lower(m, BU, BD);
+  mhd_speeds(m.alpha, m.b[K], m.gi[sym(K, K)], Gamma, Gamma / (Gamma - 1.0), P[RHO], P[PRS], dot3(vU, vD), dot3(BU, BD),
+             dot3(BU, vD), vU[K], lm, lp);
+}
+
+// a3 (second half). HLLE combination (Eq. 30; reading R6; wave speeds: reading R16)
 template <int K, int CHARGE>
 __device__ __forceinline__ void hlle(const Met& mf, double Gamma, double PL[NPRIM], double PR[NPRIM],
-                                     double sigL, double sigR, double jL, double jR, double Fh[NCONS]) {
+                                     double sigL, double sigR, double jL, double jR, int wave_mode, double rho_switch,
+                                     double Fh[NCONS]) {
   // F = (lp FL - lm FR + lp lm (UR - UL))/(lp - lm), accumulated state by state so that only one
   // state's (U, F) pair is live at a time
-  const double c = mf.alpha * sqrt(mf.gi[sym(K, K)]);
-  const double lp = fmax(0.0, c - mf.b[K]);
-  const double lm = fmin(0.0, -c - mf.b[K]);
+  limit_velocity(mf, PL);
+  limit_velocity(mf, PR);
+  double lp, lm;
+  if (wave_mode == WAVE_MHD_INSIDE && PL[RHO] > rho_switch && PR[RHO] > rho_switch) {
+    double lmL, lpL, lmR, lpR;
+    mhd_speeds_nat<K>(mf, Gamma, PL, lmL, lpL);
+    mhd_speeds_nat<K>(mf, Gamma, PR, lmR, lpR);
+    lp = fmax(0.0, fmax(lpL, lpR));
+    lm = fmin(0.0, fmin(lmL, lmR));
+  } else {
+    const double c = mf.alpha * sqrt(mf.gi[sym(K, K)]);
+    lp = fmax(0.0, c - mf.b[K]);
+    lm = fmin(0.0, -c - mf.b[K]);
+  }
   const double inv = 1.0 / (lp - lm);
   const double cL = lp * inv, cR = -lm * inv, cU = lp * lm * inv;
   double U[NCONS], F[NCONS];
-  limit_velocity(mf, PL);
   state_flux<K, CHARGE>(mf, Gamma, PL, sigL, jL, U, F);
 #pragma unroll
   for (int v = 0; v < NCONS; ++v) Fh[v] = cL * F[v] - cU * U[v];
-  limit_velocity(mf, PR);
   state_flux<K, CHARGE>(mf, Gamma, PR, sigR, jR, U, F);
 #pragma unroll
   for (int v = 0; v < NCONS; ++v) Fh[v] += cR * F[v] + cU * U[v];

@@ -122,6 +122,50 @@ __device__ __forceinline__ void half_flux(const FaceMet& m, double gog1, const d
   }
 }
 
+// A9 (reading R16) in the rotated frame: lambda-+ of the state whose rho, p, v[3], B[3] sit at xp[q * xs], q = 0, 1, 2-4,
+// 8-10; the |v| limiter of reading R4 is applied first, as half_flux does.  Returns the state's rho.
+__device__ __forceinline__ double mhd_speeds_rot(const FaceMet& m, double Gamma, const double* __restrict__ xp, int xs,
+                                                 double& lm, double& lp) {
+  const double rho = xp[0], p = xp[xs];
+  double v[3] = {xp[2 * xs], xp[3 * xs], xp[4 * xs]};
+  const double B[3] = {xp[8 * xs], xp[9 * xs], xp[10 * xs]};
+  double vD[3];
+  vD[0] = m.g[0] * v[0] + m.g[1] * v[1] + m.g[2] * v[2];
+  vD[1] = m.g[1] * v[0] + m.g[3] * v[1] + m.g[4] * v[2];
+  vD[2] = m.g[2] * v[0] + m.g[4] * v[1] + m.g[5] * v[2];
+  double vsq = v[0] * vD[0] + v[1] * vD[1] + v[2] * vD[2];
+  const double v2max = 1.0 - 1e-10;
+  if (vsq >= v2max) {
+    const double f = sqrt_fast(v2max * rcp_fast(vsq));
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { v[a] *= f; vD[a] *= f; }
+    vsq = v[0] * vD[0] + v[1] * vD[1] + v[2] * vD[2];
+  }
+  const double BD[3] = {m.g[0] * B[0] + m.g[1] * B[1] + m.g[2] * B[2], m.g[1] * B[0] + m.g[3] * B[1] + m.g[4] * B[2],
+                        m.g[2] * B[0] + m.g[4] * B[1] + m.g[5] * B[2]};
+  mhd_speeds(m.alpha, m.b0, m.gi0[0], Gamma, Gamma / (Gamma - 1.0), rho, p, vsq, B[0] * BD[0] + B[1] * BD[1] + B[2] * BD[2],
+             B[0] * vD[0] + B[1] * vD[1] + B[2] * vD[2], v[0], lm, lp);
+  return rho;
+}
+// HLLE bounds lambda-, lambda+ of a face (Eq. 30, reading R6; WAVE: PAPER.md:424, 437, reading R16)
+template <int WAVE>
+__device__ __forceinline__ void face_bounds(const GridView& G, const FaceMet& m, const double* __restrict__ plp, int pl_stride,
+                                            const double* __restrict__ prp, int pr_stride, double& lm, double& lp) {
+  if (WAVE == WAVE_MHD_INSIDE) {
+    double lmL, lpL, lmR, lpR;
+    const double rhoL = mhd_speeds_rot(m, G.Gamma, plp, pl_stride, lmL, lpL);
+    const double rhoR = mhd_speeds_rot(m, G.Gamma, prp, pr_stride, lmR, lpR);
+    if (rhoL > G.wave_rho_switch && rhoR > G.wave_rho_switch) {
+      lp = fmax(0.0, fmax(lpL, lpR));
+      lm = fmin(0.0, fmin(lmL, lmR));
+      return;
+    }
+  }
+  const double c = m.alpha * sqrt_fast(m.gi0[0]);
+  lp = fmax(0.0, c - m.b0);
+  lm = fmin(0.0, -c - m.b0);
+}
+
 // FACE_OHM only (reading R6): conductivity of a CELL from its primitives and metric
 __device__ __forceinline__ double sigma_cell(const GridView& G, long long c) {
   if (G.sigma_model == SIGMA_UNIFORM) return G.sigma0;
@@ -135,12 +179,12 @@ __device__ __forceinline__ double sigma_cell(const GridView& G, long long c) {
 
 // a3 for one face with metric m: right state PR (registers), left state read from plp (strided); F in the
 // rotated order
-template <int CHARGE, int NV>
+template <int CHARGE, int NV, int WAVE>
 __device__ __forceinline__ void riemann_m(const GridView& G, const FaceMet& m, long long cl, long long cr,
                                           const double* __restrict__ plp, int pl_stride, double PR[NVR], double Fh[NCONS]) {
   // HLLE weights (Eq. 30; reading R6)
-  const double c = m.alpha * sqrt_fast(m.gi0[0]);
-  const double lp = fmax(0.0, c - m.b0), lm = fmin(0.0, -c - m.b0);
+  double lp, lm;
+  face_bounds<WAVE>(G, m, plp, pl_stride, PR, 1, lm, lp);
   const double inv = rcp_fast(lp - lm);
   const double wL = lp * inv, wR = -lm * inv, sd = lp * lm * inv;
   double sigL = 0.0, sigR = 0.0;
@@ -157,12 +201,12 @@ __device__ __forceinline__ void riemann_m(const GridView& G, const FaceMet& m, l
 }
 // the same with both states in (shared) memory: right state at prp, left state at plp, each read just before
 // its half of the flux, so that only one state is live at a time
-template <int CHARGE, int NV>
+template <int CHARGE, int NV, int WAVE>
 __device__ __forceinline__ void riemann_mm(const GridView& G, const FaceMet& m, long long cl, long long cr,
                                            const double* __restrict__ plp, int pl_stride, const double* __restrict__ prp,
                                            int pr_stride, double Fh[NCONS]) {
-  const double c = m.alpha * sqrt_fast(m.gi0[0]);
-  const double lp = fmax(0.0, c - m.b0), lm = fmin(0.0, -c - m.b0);
+  double lp, lm;
+  face_bounds<WAVE>(G, m, plp, pl_stride, prp, pr_stride, lm, lp);
   const double inv = rcp_fast(lp - lm);
   const double wL = lp * inv, wR = -lm * inv, sd = lp * lm * inv;
   double sigL = 0.0, sigR = 0.0;
@@ -187,7 +231,8 @@ __device__ __forceinline__ void riemann(const GridView& G, const PencilTabs& T, 
                                         const double* __restrict__ plp, int pl_stride, double PR[NVR], double Fh[NCONS]) {
   FaceMet m;
   load_face_met(T, K, cl, cr, m);
-  riemann_m<CHARGE, NV>(G, m, cl, cr, plp, pl_stride, PR, Fh);
+  if (G.wave_mode == WAVE_MHD_INSIDE) riemann_m<CHARGE, NV, WAVE_MHD_INSIDE>(G, m, cl, cr, plp, pl_stride, PR, Fh);
+  else riemann_m<CHARGE, NV, WAVE_LIGHT>(G, m, cl, cr, plp, pl_stride, PR, Fh);
 }
 inline PencilTabs make_tabs(const GridView& G) {
   PencilTabs T;

@@ -57,7 +57,7 @@ __device__ __forceinline__ void face_flux(const GridView& G, long long cR, doubl
     lower(mc, vU, vD);
     sigR = sigma_of(G, G.P[RHO][cR] * (1.0 / sqrt(1.0 - dot3(vU, vD))), cR);
   }
-  hlle<K, CHARGE>(mf, G.Gamma, PL, PR, sigL, sigR, jL, jR, Fh);
+  hlle<K, CHARGE>(mf, G.Gamma, PL, PR, sigL, sigR, jL, jR, G.wave_mode, G.wave_rho_switch, Fh);
 }
 
 // a5 (flux-divergence part; the point-wise part is stage_precombine in rgrmhd_sources.cuh).  dU = -div F of the

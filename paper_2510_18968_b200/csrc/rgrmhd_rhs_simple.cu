@@ -141,12 +141,66 @@ cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, 
 }
 
 // ------------------------------------------------------------------------------------------------
+// A22. charge mode DIV_E (reading R15): q = nabla_i E^i = d_i(sqrt(gamma) E^i)/sqrt(gamma) of the
+// stage, second-order centred differences (inactive directions dropped), from the ghost-filled stage primitives.
+// Writes q into P and applies the two explicit source terms that carry the charge,
+//   S(calE^i) -= alpha calQ v^i,   S(Psi) += alpha calQ            (Eq. 27 / reading R1),
+// to the bracket of the next stage vector (STAGE 1: U*2 += dt ...; STAGE 2: U^{n+1} += dt/2 ...);
+// STAGE 3 (new state, on output): q and calQ = sqrt(gamma) q only.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double sqrtg_cell(const GridView& G, long long c) {
+  const double gxx = __ldg(G.met[MGXX] + c), gxy = __ldg(G.met[MGXY] + c), gxz = __ldg(G.met[MGXZ] + c);
+  const double gyy = __ldg(G.met[MGYY] + c), gyz = __ldg(G.met[MGYZ] + c), gzz = __ldg(G.met[MGZZ] + c);
+  return sqrt(gxx * (gyy * gzz - gyz * gyz) + gxy * (gxz * gyz - gxy * gzz) + gxz * (gxy * gyz - gxz * gyy));
+}
+
+template <int STAGE>
+__global__ void __launch_bounds__(128)
+k_charge_div_e(const __grid_constant__ GridView G, double dt) {
+  const int nx = G.n[0], ny = G.n[1];
+  const long long nint = (long long)nx * ny * G.n[2];
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nint) return;
+  const int i = (int)(t % nx);
+  const long long r = t / nx;
+  const long long c = cell_index(G, i, (int)(r % ny), (int)(r / ny));
+  double div = 0.0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    if (G.n[d] > 1) {
+      const long long s = G.stride[d];
+      div += (sqrtg_cell(G, c + s) * G.P[EX + d][c + s] - sqrtg_cell(G, c - s) * G.P[EX + d][c - s]) * (0.5 * G.inv_dx[d]);
+    }
+  }
+  G.P[QCH][c] = div / sqrtg_cell(G, c);
+  if (STAGE == 3) {
+    G.Un[CQ][c] = div;
+  } else {
+    const double w = (STAGE == 1) ? dt : 0.5 * dt, aq = __ldg(G.met[MALP] + c) * div;
+    double* const* T = (STAGE == 1) ? G.Us : G.Un;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) T[CEX + a][c] -= w * aq * G.P[VX + a][c];
+    T[CPSI][c] += w * aq;
+  }
+}
+
+cudaError_t launch_charge_div_e(const GridView& G, int stage, double dt, cudaStream_t st) {
+  const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
+  const int threads = 128;
+  const unsigned blocks = (unsigned)((nint + threads - 1) / threads);
+  if (stage == 1) k_charge_div_e<1><<<blocks, threads, 0, st>>>(G, dt);
+  else if (stage == 2) k_charge_div_e<2><<<blocks, threads, 0, st>>>(G, dt);
+  else k_charge_div_e<3><<<blocks, threads, 0, st>>>(G, dt);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
 // a7. max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k
 // (Eq. 30; reading R14): warp shuffle -> block -> one atomicMax on the bit pattern
 // (non-negative doubles order like unsigned integers).
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_max_speed(const __grid_constant__ GridView G, unsigned long long* __restrict__ out) {
+k_max_speed(const __grid_constant__ GridView G, unsigned long long* __restrict__ out, bool mhd_mode) {
   const int nx = G.n[0], ny = G.n[1];
   const long long nint = (long long)nx * ny * G.n[2];
   double mx = 0.0;
@@ -155,10 +209,24 @@ k_max_speed(const __grid_constant__ GridView G, unsigned long long* __restrict__
     const long long r = t / nx;
     const int j = (int)(r % ny), k = (int)(r / ny);
     Met m;
-    load_met_cell(G, cell_index(G, i, j, k), m);
+    const long long c = cell_index(G, i, j, k);
+    load_met_cell(G, c, m);
+    if (mhd_mode && G.P[RHO][c] > G.wave_rho_switch) {   // A9: the cell's own ideal-GRMHD speeds (reading R16)
+      double P[NPRIM];
 #pragma unroll
-    for (int d = 0; d < 3; ++d)
-      if (G.n[d] > 1) mx = fmax(mx, (m.alpha * sqrt(m.gi[sym(d, d)]) + fabs(m.b[d])) * G.inv_dx[d]);
+      for (int v = 0; v < NPRIM; ++v) P[v] = (v <= VZ || (v >= BX && v <= BZ)) ? G.P[v][c] : 0.0;
+      double lm[3], lp[3];
+      mhd_speeds_nat<0>(m, G.Gamma, P, lm[0], lp[0]);
+      mhd_speeds_nat<1>(m, G.Gamma, P, lm[1], lp[1]);
+      mhd_speeds_nat<2>(m, G.Gamma, P, lm[2], lp[2]);
+#pragma unroll
+      for (int d = 0; d < 3; ++d)
+        if (G.n[d] > 1) mx = fmax(mx, fmax(fabs(lm[d]), fabs(lp[d])) * G.inv_dx[d]);
+    } else {
+#pragma unroll
+      for (int d = 0; d < 3; ++d)
+        if (G.n[d] > 1) mx = fmax(mx, (m.alpha * sqrt(m.gi[sym(d, d)]) + fabs(m.b[d])) * G.inv_dx[d]);
+    }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
@@ -171,12 +239,12 @@ k_max_speed(const __grid_constant__ GridView G, unsigned long long* __restrict__
   }
 }
 
-cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, int sm_count, cudaStream_t st) {
+cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, bool have_prims, int sm_count, cudaStream_t st) {
   const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
   const int threads = 256;
   long long blocks = (nint + threads - 1) / threads;
   if (blocks > (long long)sm_count * 8) blocks = (long long)sm_count * 8;   // 8 resident 256-thread CTAs per SM
-  k_max_speed<<<(unsigned)blocks, threads, 0, st>>>(G, out);
+  k_max_speed<<<(unsigned)blocks, threads, 0, st>>>(G, out, G.wave_mode == WAVE_MHD_INSIDE && have_prims);
   return cudaGetLastError();
 }
 

@@ -126,7 +126,7 @@ __device__ __forceinline__ void lds_stencil(const double* __restrict__ p, int s,
 }
 }  // namespace
 
-template <int RECON, int CHARGE, int STAGE>
+template <int RECON, int CHARGE, int STAGE, int WAVE>
 // 168 registers: 12 warps sit 3 + 3 + 3 + 3 on the four schedulers, each with a 16 K-register file
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTabs T,
@@ -211,7 +211,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
           for (int vr = 0; vr < NV; ++vr) PR[vr] = S.exlo[vr][r];
           FaceMet m;
           finish_face_met(raw, m);
-          riemann_m<CHARGE, NV>(G, m, cl, cr, &S.exhi[0][r], 16, PR, F);
+          riemann_m<CHARGE, NV, WAVE>(G, m, cl, cr, &S.exhi[0][r], 16, PR, F);
           const int dst = (K == 0) ? r * EXW + txn : tyn * EXW + r;
 #pragma unroll
           for (int v = 0; v < NCONS; ++v) S.fx[T.nat[K][v]][dst] = F[v];
@@ -419,7 +419,7 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
         // the left states are read from shared memory inside, after the right state's half of the flux
         const double* pl = (K == 2) ? &S.chi[0][tid] : &S.ex[0][base];
         const int pls = (K == 2) ? NT : EXP;
-        riemann_mm<CHARGE, NV>(G, m, cl, cr, pl, pls, &S.los[0][tid], NT, F);
+        riemann_mm<CHARGE, NV, WAVE>(G, m, cl, cr, pl, pls, &S.los[0][tid], NT, F);
       }
       if (K < 2) {
         if (solve) {
@@ -517,22 +517,26 @@ static int choose_cz(const GridView& G, int sm_count) {
   return best;
 }
 
-template <int RECON, int CHARGE, int STAGE>
+template <int RECON, int CHARGE, int STAGE, int WAVE>
 static cudaError_t launch_one(const GridView& G, const TmaMaps& M, double dt, int sm_count, cudaStream_t st) {
   const int cz = choose_cz(G, sm_count);
   const PencilTabs T = make_tabs(G);
   dim3 block(NTHREADS, 1, 1);
   dim3 grid((G.n[0] + TX - 1) / TX, (G.n[1] + TY - 1) / TY, (G.n[2] + cz - 1) / cz);
   const size_t smem = sizeof(Smem);
-  cudaError_t e = cudaFuncSetAttribute(k_flux_tma<RECON, CHARGE, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(k_flux_tma<RECON, CHARGE, STAGE, WAVE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_flux_tma<RECON, CHARGE, STAGE><<<grid, block, smem, st>>>(G, T, M, dt, cz);
+  k_flux_tma<RECON, CHARGE, STAGE, WAVE><<<grid, block, smem, st>>>(G, T, M, dt, cz);
   return cudaGetLastError();
 }
 
 template <int RECON, int CHARGE>
 static cudaError_t launch_rc(const GridView& G, const TmaMaps& M, double dt, int stage, int sm_count, cudaStream_t st) {
-  return stage == 1 ? launch_one<RECON, CHARGE, 1>(G, M, dt, sm_count, st) : launch_one<RECON, CHARGE, 2>(G, M, dt, sm_count, st);
+  if (G.wave_mode == WAVE_MHD_INSIDE)
+    return stage == 1 ? launch_one<RECON, CHARGE, 1, WAVE_MHD_INSIDE>(G, M, dt, sm_count, st)
+                      : launch_one<RECON, CHARGE, 2, WAVE_MHD_INSIDE>(G, M, dt, sm_count, st);
+  return stage == 1 ? launch_one<RECON, CHARGE, 1, WAVE_LIGHT>(G, M, dt, sm_count, st)
+                    : launch_one<RECON, CHARGE, 2, WAVE_LIGHT>(G, M, dt, sm_count, st);
 }
 
 cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int stage, int recon, int sm_count, cudaStream_t st) {

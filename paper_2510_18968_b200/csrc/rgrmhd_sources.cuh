@@ -102,7 +102,9 @@ __device__ __forceinline__ void add_sources(const GridView& G, const Met& m, con
   raise(m, SD, SU);
   const double tauD = sg * (hW2 - p + pem);                                         // tau + D (Eq. 22-23)
   const double cE[3] = {sg * EU[0], sg * EU[1], sg * EU[2]}, cB[3] = {sg * BU[0], sg * BU[1], sg * BU[2]};
-  const double cPsi = sg * P[PSI], cPhi = sg * P[PHI], cQ = sg * P[QCH];
+  // charge mode DIV_E: the stage's charge is computed from its electric field AFTER this kernel
+  // (k_charge_div_e), which also applies the two source terms that carry it
+  const double cPsi = sg * P[PSI], cPhi = sg * P[PHI], cQ = (G.charge_mode == CHARGE_DIV_E) ? 0.0 : sg * P[QCH];
   const double asg = al * sg;
   {
     double t1 = 0.0;

@@ -51,6 +51,7 @@ BC_PERIODIC, BC_OUTFLOW = 0, 1
 SIGMA_UNIFORM, SIGMA_ARRAY, SIGMA_POWER_D, SIGMA_ATMO = 0, 1, 2, 3
 RECON_MINMOD, RECON_MC, RECON_WENO5 = 0, 1, 2
 CHARGE_FACE_OHM, CHARGE_CELL_CURRENT, CHARGE_DIV_E = 0, 1, 2
+WAVE_LIGHT, WAVE_MHD_INSIDE = 0, 1
 
 
 def splitmix64_uniform(seed: int, idx: np.ndarray) -> np.ndarray:

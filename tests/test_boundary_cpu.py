@@ -78,7 +78,8 @@ def test_enum_values_mirrored_in_workloads():
     src = open(HEADER).read()
     vals = dict((k, int(v)) for k, v in re.findall(r"\b(RGRMHD_[A-Z0-9_]+)\s*=\s*(-?\d+)\b(?!\s*<<)", src))
     for k in ("BC_PERIODIC", "BC_OUTFLOW", "SIGMA_UNIFORM", "SIGMA_ARRAY", "SIGMA_POWER_D", "SIGMA_ATMO",
-              "RECON_MINMOD", "RECON_MC", "RECON_WENO5", "CHARGE_FACE_OHM", "CHARGE_CELL_CURRENT", "CHARGE_DIV_E"):
+              "RECON_MINMOD", "RECON_MC", "RECON_WENO5", "CHARGE_FACE_OHM", "CHARGE_CELL_CURRENT", "CHARGE_DIV_E",
+              "WAVE_LIGHT", "WAVE_MHD_INSIDE"):
         assert vals["RGRMHD_" + k] == getattr(wl, k), k
 
 

@@ -365,8 +365,8 @@ def test_api_errors(binding):
     assert L.rgrmhd_create(C.byref(h), C.byref(p)) == -1
     p.ng = 3; p.gamma_eos = 1.0
     assert L.rgrmhd_create(C.byref(h), C.byref(p)) == -1
-    p.gamma_eos = 2.0; p.charge_mode = 2
-    assert L.rgrmhd_create(C.byref(h), C.byref(p)) == -1          # DIV_E not built
+    p.gamma_eos = 2.0; p.charge_mode = 3
+    assert L.rgrmhd_create(C.byref(h), C.byref(p)) == -1          # unknown charge mode
     p.charge_mode = 1; p.dx[0] = 0.0
     assert L.rgrmhd_create(C.byref(h), C.byref(p)) == -1
     p.dx[0] = 0.1

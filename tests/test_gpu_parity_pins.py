@@ -204,3 +204,48 @@ def test_face_fixup_stencil(binding, variant):
         for _ in range(4):
             g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
         _compare(g, o, n, 0.1, TOL20, "fix-up stencil 5 steps n=%s" % (n,))
+
+
+# ----------------------------------------------------------------------------------------------
+# charge mode C: q = nabla_i E^i
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_charge_mode_div_e(binding, variant):
+    """Curved periodic block (shift, K_ij, off-diagonal metric), a config-4 sub-block with outflow walls, and a 1D
+    block: the charge of every stage and of the new state comes from the centred divergence of calE."""
+    from test_oracle_scheme import _pad_periodic, _periodic_problem
+    rng = np.random.default_rng(17)
+    n = (38, 21, 9)
+    metric, P = _periodic_problem(40, rng, True)
+    sl = (slice(None), slice(0, n[2]), slice(0, n[1]), slice(0, n[0]))
+    metric, P = _pad_periodic(np.ascontiguousarray(metric[sl])), _pad_periodic(np.ascontiguousarray(P[sl]))
+    par = dict(n=n, dx=(1 / 40,) * 3, bc=(0, 0, 0), gamma_eos=5 / 3, sigma_model=0, sigma0=30.0, kappa=1.0,
+               charge_mode=wl.CHARGE_DIV_E)
+    g, o = _both(binding, par, metric, P, variant)
+    dt = 0.2 / 40
+    g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+    _compare(g, o, n, 1 / 40, TOL1, "div E 1 step")
+    for s in range(4):
+        g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+        if s == 1:
+            g.stats()                        # flushes the pending recovery mid-run: the charge is still due on output
+    _compare(g, o, n, 1 / 40, TOL20, "div E 5 steps")
+    w = wl.blast_curved()
+    nb, bc = (40, 36, 20), (wl.BC_OUTFLOW,) * 3
+    f = w.fields((120, 138, 100), nb)
+    o = oracle.from_workload(w, fields=f, omp=True, n=nb, bc=bc, charge_mode=wl.CHARGE_DIV_E)
+    g = binding.from_workload(w, fields=f, n=nb, bc=bc, charge_mode=wl.CHARGE_DIV_E)
+    g.set_rhs_variant(variant)
+    for _ in range(20):
+        g.step(w.dt, w.recon); o.step(w.dt, w.recon)
+    _compare(g, o, nb, w.dx[0], TOL20, "div E cfg4 block 20 steps")
+    assert g.stats()["c2p_failures"] == 0
+    w1 = wl.shocktube(n=64, sigma0=1e3)
+    f1 = w1.fields()
+    f1["prims"][wl.BZ] = 0.3                                     # non-coplanar: the charge sector is live
+    o = oracle.from_workload(w1, fields=f1, charge_mode=wl.CHARGE_DIV_E)
+    g = binding.from_workload(w1, fields=f1, charge_mode=wl.CHARGE_DIV_E)
+    for _ in range(10):
+        g.step(w1.dt, wl.RECON_MC); o.step(w1.dt, wl.RECON_MC)
+    _compare(g, o, w1.n, w1.dx[0], TOL20, "div E 1D")
+    assert np.abs(interior(g.get_prims(), w1.n)[13]).max() > 1e-3
