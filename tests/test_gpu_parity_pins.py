@@ -249,3 +249,54 @@ def test_charge_mode_div_e(binding, variant):
         g.step(w1.dt, wl.RECON_MC); o.step(w1.dt, wl.RECON_MC)
     _compare(g, o, w1.n, w1.dx[0], TOL20, "div E 1D")
     assert np.abs(interior(g.get_prims(), w1.n)[13]).max() > 1e-3
+
+
+# ----------------------------------------------------------------------------------------------
+# f1: state-dependent HLLE wave speeds
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_wave_speed_mode_mhd_inside(binding, variant):
+    """Ideal-GRMHD characteristic speeds where both face states are denser than the switch, light speed elsewhere:
+    (i) a curved periodic block with every state 'inside' (shift, K_ij, off-diagonal metric; even and odd row pitch),
+    (ii) the config-5 block across the stellar surface, where the switch separates star and atmosphere;
+    the CFL reduction becomes a per-step, state-dependent one and must agree too."""
+    from test_oracle_scheme import _pad_periodic, _periodic_problem
+    rng = np.random.default_rng(23)
+    for n in ((38, 21, 9), (37, 11, 9)):
+        metric, P = _periodic_problem(40, rng, True)
+        sl = (slice(None), slice(0, n[2]), slice(0, n[1]), slice(0, n[0]))
+        metric, P = _pad_periodic(np.ascontiguousarray(metric[sl])), _pad_periodic(np.ascontiguousarray(P[sl]))
+        for switch in (0.0, 1.0):                      # everything inside / the switch cuts through the data (rho ~ 1 +- 0.2)
+            par = dict(n=n, dx=(1 / 40,) * 3, bc=(0, 0, 0), gamma_eos=5 / 3, sigma_model=0, sigma0=30.0, kappa=1.0,
+                       wave_speed_mode=wl.WAVE_MHD_INSIDE, wave_rho_switch=switch)
+            g, o = _both(binding, par, metric, P, variant)
+            assert abs(g.max_speed() - o.max_speed()) <= 1e-14 * o.max_speed()
+            dt = 0.2 / 40
+            g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+            _compare(g, o, n, 1 / 40, TOL1, "mhd speeds 1 step")
+            for _ in range(4):
+                g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+            _compare(g, o, n, 1 / 40, TOL20, "mhd speeds 5 steps")
+            ms_g, ms_o = g.max_speed(), o.max_speed()                # pending final recovery is flushed first
+            assert abs(ms_g - ms_o) <= 1e-12 * ms_o
+    w = wl.tov_like()
+    i_surf = int(round((8.125 + 12.0) / w.dx[0]))
+    nb, bc = (40, 12, 10), (wl.BC_OUTFLOW,) * 3
+    f = w.fields((i_surf - 20, 256 - 6, 256 - 5), nb)
+    over = dict(wave_speed_mode=wl.WAVE_MHD_INSIDE, wave_rho_switch=1e-9)
+    o = oracle.from_workload(w, fields=f, omp=True, n=nb, bc=bc, **over)
+    g = binding.from_workload(w, fields=f, n=nb, bc=bc, **over)
+    g.set_rhs_variant(variant)
+    for _ in range(10):
+        g.step(w.dt, w.recon); o.step(w.dt, w.recon)
+    _compare(g, o, nb, w.dx[0], TOL20, "mhd speeds cfg5 block")
+    assert g.stats()["floor_resets"] == o.stats()["floor_resets"] > 0
+    # the result differs from the light-speed solver (the mode is live), and a switch nothing exceeds is bit-identical to it
+    gl = binding.from_workload(w, fields=f, n=nb, bc=bc)
+    goff = binding.from_workload(w, fields=f, n=nb, bc=bc, wave_speed_mode=wl.WAVE_MHD_INSIDE, wave_rho_switch=1e30)
+    for h in (gl, goff):
+        h.set_rhs_variant(variant)
+        for _ in range(10):
+            h.step(w.dt, w.recon)
+    assert np.array_equal(gl.get_prims(), goff.get_prims())
+    assert not np.array_equal(gl.get_prims(), g.get_prims())
