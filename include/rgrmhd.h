@@ -77,7 +77,13 @@ enum { RGRMHD_WAVE_LIGHT = 0, RGRMHD_WAVE_MHD_INSIDE = 1 };
 
 /* `scheme` argument of rgrmhd_step = reconstruction | time scheme */
 enum { RGRMHD_RECON_MINMOD = 0, RGRMHD_RECON_MC = 1, RGRMHD_RECON_WENO5 = 2, RGRMHD_RECON_MASK = 0xff };
-enum { RGRMHD_TIME_IMEX_SSP2_222 = 0 << 8, RGRMHD_TIME_MASK = 0xff00 };
+/* time schemes: the IMEX-RK SSP schemes the paper incorporates.  SSP2_222 (Eq. 35-37, Table I) is the
+ * paper's production scheme and this library's tuned path (6 launches per step, deferred final recovery); the others
+ * run through the general double-Butcher-tableau driver of Eq. 32-34 (one point-wise kernel per stage plus one for the
+ * new state, one flux kernel per stage whose F is used); SSP2_222_GENERAL is the production scheme through that
+ * driver (a cross-check: same result to round-off). */
+enum { RGRMHD_TIME_IMEX_SSP2_222 = 0 << 8, RGRMHD_TIME_IMEX_SSP2_332 = 1 << 8, RGRMHD_TIME_IMEX_SSP3_332 = 2 << 8,
+       RGRMHD_TIME_IMEX_SSP3_433 = 3 << 8, RGRMHD_TIME_IMEX_SSP2_222_GENERAL = 4 << 8, RGRMHD_TIME_MASK = 0xff00 };
 
 typedef struct {
   int    n[3];        /* interior cells per direction; n = 1 marks an inactive direction          */
@@ -133,9 +139,10 @@ int rgrmhd_set_sigma(rgrmhd_t h, const double* sigma);
  * the conserved state (Eq. 22-24, 28).  Requires set_metric first. */
 int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]);
 
-/* One IMEX-SSP2(2,2,2) step of size dt (Eq. 35-37): implicit-E + recovery (+ the point-wise
- * explicit sources and stage-combine terms of that stage), ghost fill, reconstruction + HLLE +
- * flux divergence (an increment the next recovery adds to its stage vector); twice; final recovery. */
+/* One IMEX-RK step of size dt.  scheme = RGRMHD_RECON_* | RGRMHD_TIME_*.  SSP2(2,2,2) (Eq. 35-37): implicit-E +
+ * recovery (+ the point-wise explicit sources and stage-combine terms of that stage), ghost fill, reconstruction +
+ * HLLE + flux divergence (an increment the next recovery adds to its stage vector); twice; final recovery.  The
+ * other schemes: the same kernels stage by stage (Eq. 32); the first 3-/4-stage step allocates 28 more fields. */
 int rgrmhd_step(rgrmhd_t h, double dt, int scheme);
 
 /* rgrmhd_step enqueues everything of its step except the final recovery P^{n+1} = recovery(U^{n+1}) (Eq. 37,

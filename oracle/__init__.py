@@ -241,6 +241,16 @@ def wave_speeds_point(P, k, gamma_eos, alpha=1.0, beta=None, g6=None):
     return lm.value, lp.value
 
 
+def tableau(time_scheme: int):
+    """(s, At, wt, A, w) of the oracle's double Butcher tableau for a time scheme (0..4), cut to s stages."""
+    At, A = np.zeros((4, 4)), np.zeros((4, 4))
+    wt, w = np.zeros(4), np.zeros(4)
+    s = lib().oracle_tableau(int(time_scheme), _dp(At), _dp(wt), _dp(A), _dp(w))
+    if s < 0:
+        raise ValueError("unknown time scheme")
+    return s, At[:s, :s], wt[:s], A[:s, :s], w[:s]
+
+
 def sigma_point(model, sigma0, sigma_exp, sigma_dref, Dhat, sigma_cell=0.0):
     return lib().oracle_sigma_point(int(model), float(sigma0), float(sigma_exp), float(sigma_dref), float(Dhat),
                                     float(sigma_cell))

@@ -1027,6 +1027,104 @@ void step(Grid& G, double dt, int scheme) {
   final_charge(G);
 }
 
+// ---------------------------------------------------------------------------------------------
+// A12. the other IMEX-RK SSP schemes the paper incorporates: SSP2(3,3,2), SSP3(3,3,2), SSP3(4,3,3),
+// through the GENERAL form Eq. 32 with a double Butcher tableau (Eq. 33-34).  PAPER.md does not
+// print these tableaux (refs [19], [31]); the coefficients below are the published Pareschi-Russo ones, PINNED by
+// the order conditions they must satisfy (tests/test_oracle_imex_tableaux.py), not by trust.
+//   U^(i)   = U^n + dt sum_{j<i} at_ij F[U^(j)] + dt sum_{j<=i} a_ij R[U^(j)]
+//   U^{n+1} = U^n + dt sum_i wt_i F[U^(i)] + dt sum_i w_i R[U^(i)]
+// with the split of PAPER.md:216 (R acts on X = calE only) and R^(i) = (X^(i) - X*^(i))/(a_ii dt) (reading R11),
+// X*^(i) = the explicit part of the stage vector; the recovery of U^{n+1} at fixed calE (reading R12).
+// A stage whose F is used by nobody (zero column in At and zero weight) is not evaluated.
+// ---------------------------------------------------------------------------------------------
+struct Tableau { int s; double At[4][4], wt[4], A[4][4], w[4]; };
+enum { TIME_SSP2_222 = 0, TIME_SSP2_332 = 1, TIME_SSP3_332 = 2, TIME_SSP3_433 = 3, TIME_SSP2_222_GENERAL = 4 };
+
+bool tableau_of(int time_scheme, Tableau& T) {
+  std::memset(&T, 0, sizeof(T));
+  const double g = 1.0 - 1.0 / std::sqrt(2.0);
+  switch (time_scheme) {
+    case TIME_SSP2_222: case TIME_SSP2_222_GENERAL:          // Eq. 35-37 / Table I
+      T.s = 2;
+      T.At[1][0] = 1.0; T.wt[0] = T.wt[1] = 0.5;
+      T.A[0][0] = g; T.A[1][0] = 1.0 - 2.0 * g; T.A[1][1] = g; T.w[0] = T.w[1] = 0.5;
+      return true;
+    case TIME_SSP2_332:                                      // stiffly accurate, second order
+      T.s = 3;
+      T.At[1][0] = 0.5; T.At[2][0] = 0.5; T.At[2][1] = 0.5; T.wt[0] = T.wt[1] = T.wt[2] = 1.0 / 3.0;
+      T.A[0][0] = 0.25; T.A[1][1] = 0.25; T.A[2][0] = T.A[2][1] = T.A[2][2] = 1.0 / 3.0;
+      T.w[0] = T.w[1] = T.w[2] = 1.0 / 3.0;
+      return true;
+    case TIME_SSP3_332:                                      // third-order SSP explicit part, second order overall
+      T.s = 3;
+      T.At[1][0] = 1.0; T.At[2][0] = 0.25; T.At[2][1] = 0.25; T.wt[0] = T.wt[1] = 1.0 / 6.0; T.wt[2] = 2.0 / 3.0;
+      T.A[0][0] = g; T.A[1][0] = 1.0 - 2.0 * g; T.A[1][1] = g; T.A[2][0] = 0.5 - g; T.A[2][2] = g;
+      T.w[0] = T.w[1] = 1.0 / 6.0; T.w[2] = 2.0 / 3.0;
+      return true;
+    case TIME_SSP3_433: {                                    // third order
+      const double al = 0.24169426078821, be = 0.06042356519705, et = 0.12915286960590;
+      T.s = 4;
+      T.At[2][1] = 1.0; T.At[3][1] = 0.25; T.At[3][2] = 0.25; T.wt[1] = T.wt[2] = 1.0 / 6.0; T.wt[3] = 2.0 / 3.0;
+      T.A[0][0] = al; T.A[1][0] = -al; T.A[1][1] = al; T.A[2][1] = 1.0 - al; T.A[2][2] = al;
+      T.A[3][0] = be; T.A[3][1] = et; T.A[3][2] = 0.5 - be - et - al; T.A[3][3] = al;
+      T.w[1] = T.w[2] = 1.0 / 6.0; T.w[3] = 2.0 / 3.0;
+      return true;
+    }
+  }
+  return false;
+}
+
+void step_tableau(Grid& G, double dt, int scheme, const Tableau& T) {
+  const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2], s = T.s;
+  std::vector<double> F[4][NCONS], R[4][3], Xst[3], Xi[3];
+  for (int q = 0; q < 3; ++q) { Xst[q].assign(G.ntot, 0.0); Xi[q].assign(G.ntot, 0.0); }
+  for (int i = 0; i < s; ++i) {
+    for (int q = 0; q < 3; ++q) R[i][q].assign(G.ntot, 0.0);
+    // stage vector: explicit part (its calE entries are X*^(i)) ...
+#pragma omp parallel for collapse(3) schedule(static)
+    for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int ii = 0; ii < nx; ++ii) {
+      const long c = G.idx(ii, j, k);
+      for (int v = 0; v < NCONS; ++v) {
+        double u = G.Un[v][c];
+        for (int jj = 0; jj < i; ++jj) if (T.At[i][jj] != 0.0) u += dt * T.At[i][jj] * F[jj][v][c];
+        G.Us[v][c] = u;
+      }
+      for (int q = 0; q < 3; ++q) {
+        double x = G.Us[CEX + q][c];
+        for (int jj = 0; jj < i; ++jj) if (T.A[i][jj] != 0.0) x += dt * T.A[i][jj] * R[jj][q][c];
+        G.Us[CEX + q][c] = x;
+        Xst[q][c] = x;
+      }
+    }
+    // ... and its implicit part: solve for (calE^(i), P^(i)) with a = a_ii dt
+    solve_all(G, G.Us, T.A[i][i] * dt, Xi, false);
+#pragma omp parallel for collapse(3) schedule(static)
+    for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int ii = 0; ii < nx; ++ii) {
+      const long c = G.idx(ii, j, k);
+      for (int q = 0; q < 3; ++q) R[i][q][c] = (Xi[q][c] - Xst[q][c]) / (T.A[i][i] * dt);
+    }
+    bool used = T.wt[i] != 0.0;
+    for (int jj = i + 1; jj < s; ++jj) used = used || T.At[jj][i] != 0.0;
+    if (!used) continue;
+    stage_ghosts_and_charge(G);
+    for (int v = 0; v < NCONS; ++v) F[i][v].assign(G.ntot, 0.0);
+    rhs_all(G, scheme, F[i]);
+  }
+#pragma omp parallel for collapse(3) schedule(static)
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int ii = 0; ii < nx; ++ii) {
+    const long c = G.idx(ii, j, k);
+    for (int v = 0; v < NCONS; ++v) {
+      double u = G.Un[v][c];
+      for (int i = 0; i < s; ++i) if (T.wt[i] != 0.0) u += dt * T.wt[i] * F[i][v][c];
+      if (v >= CEX && v <= CEZ) for (int i = 0; i < s; ++i) if (T.w[i] != 0.0) u += dt * T.w[i] * R[i][v - CEX][c];
+      G.Un[v][c] = u;
+    }
+  }
+  solve_all(G, G.Un, 0.0, nullptr, true);
+  final_charge(G);
+}
+
 // a7. max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k (Eq. 30); with
 // wave_speed_mode MHD_INSIDE (A9) the cell's own max(|lambda-|, |lambda+|)/dx^k where rho > wave_rho_switch
 double max_speed(const Grid& G) {
@@ -1142,9 +1240,11 @@ int oracle_step(void* h, double dt, int scheme) {
   Grid* G = (Grid*)h;
   if (!G || !(dt > 0.0)) return -1;
   if (!G->have_metric || !G->have_prims || (G->par.sigma_model == SIGMA_ARRAY && !G->have_sigma)) return -2;
-  const int recon = scheme & 0xff;
-  if (recon < 0 || recon > 2 || (scheme & 0xff00) != 0) return -1;
-  step(*G, dt, recon);
+  const int recon = scheme & 0xff, time_scheme = (scheme >> 8) & 0xff;
+  Tableau T;
+  if (recon < 0 || recon > 2 || (scheme & ~0xffff) != 0 || !tableau_of(time_scheme, T)) return -1;
+  if (time_scheme == TIME_SSP2_222) step(*G, dt, recon);      // Eq. 35-37 written out
+  else step_tableau(*G, dt, recon, T);                        // Eq. 32 with the scheme's tableau
   return 0;
 }
 int oracle_max_speed(void* h, double* out) {
@@ -1261,6 +1361,13 @@ int oracle_wave_speeds_point(double Gamma, double alpha, const double* beta3, co
   Metric m = metric_from_arrays(alpha, beta3, g6);
   mhd_wave_speeds(m, Gamma, k, P, lam_minus, lam_plus);
   return 0;
+}
+// the double Butcher tableau of a time scheme: s, then At, wt, A, w as 4x4 / 4 arrays (row major); returns s or -1
+int oracle_tableau(int time_scheme, double* At, double* wt, double* A, double* w) {
+  Tableau T;
+  if (!tableau_of(time_scheme, T)) return -1;
+  for (int i = 0; i < 4; ++i) { wt[i] = T.wt[i]; w[i] = T.w[i]; for (int j = 0; j < 4; ++j) { At[4 * i + j] = T.At[i][j]; A[4 * i + j] = T.A[i][j]; } }
+  return T.s;
 }
 // conductivity models at one point (A18)
 double oracle_sigma_point(int model, double sigma0, double sigma_exp, double sigma_dref, double Dhat, double sigma_cell) {

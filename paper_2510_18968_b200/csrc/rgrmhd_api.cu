@@ -27,12 +27,24 @@ cudaError_t launch_charge_div_e(const GridView& G, int stage, double dt, cudaStr
 cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, bool have_prims, int sm_count, cudaStream_t st);
 }  // namespace rg
 
+namespace rg {
+struct AccTab { double* f[NCONS]; };
+struct StageGen {           // mirrors rgrmhd_imex_gen.cu
+  int stage, nstages, use_dprev, init;
+  double aii, w_dprev[5], w_src[5], w_stiff[5];
+  AccTab acc[5];
+};
+cudaError_t launch_stage_gen(const GridView& G, const StageGen& W, double dt, StatsDev* stats, cudaStream_t st);
+cudaError_t launch_charge_sources_gen(const GridView& G, const StageGen& W, double dt, cudaStream_t st);
+}  // namespace rg
+
 struct rgrmhd_s {
   rgrmhd_params par;
   rg::GridView G;
   int device = 0;
   cudaStream_t stream = nullptr;
   double* slab = nullptr;            // all fields, one allocation
+  double* slab2 = nullptr;           // accumulators of the 3rd / 4th stage of the general tableau driver (allocated on first use)
   long long field_stride = 0;        // doubles between consecutive fields (ntot rounded up to 32)
   rg::StatsDev* stats_dev = nullptr;
   unsigned long long* maxspeed_dev = nullptr;
@@ -195,6 +207,7 @@ int rgrmhd_destroy(rgrmhd_t h) {
     cudaStreamSynchronize(h->stream);
     for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(h->slab);
+    cudaFree(h->slab2);
     cudaFree(h->stats_dev);
     rg::tma_destroy(h->tma);
   }
@@ -348,12 +361,134 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]) {
   return RGRMHD_OK;
 }
 
+// ---- general IMEX-RK driver (Eq. 32-34) ---------------------------------
+namespace {
+struct Tableau { int s; double At[4][4], wt[4], A[4][4], w[4]; };
+
+// The schemes the paper incorporates.  PAPER.md prints only Table I's scheme (through Eq. 35-37); the
+// others are the published Pareschi-Russo tableaux, checked against the IMEX order conditions by the tests.
+bool tableau_of(int time_scheme, Tableau& T) {
+  std::memset(&T, 0, sizeof(T));
+  const double g = 1.0 - 1.0 / std::sqrt(2.0);
+  switch (time_scheme) {
+    case RGRMHD_TIME_IMEX_SSP2_222_GENERAL:
+      T.s = 2;
+      T.At[1][0] = 1.0; T.wt[0] = T.wt[1] = 0.5;
+      T.A[0][0] = g; T.A[1][0] = 1.0 - 2.0 * g; T.A[1][1] = g; T.w[0] = T.w[1] = 0.5;
+      return true;
+    case RGRMHD_TIME_IMEX_SSP2_332:
+      T.s = 3;
+      T.At[1][0] = 0.5; T.At[2][0] = 0.5; T.At[2][1] = 0.5; T.wt[0] = T.wt[1] = T.wt[2] = 1.0 / 3.0;
+      T.A[0][0] = 0.25; T.A[1][1] = 0.25; T.A[2][0] = T.A[2][1] = T.A[2][2] = 1.0 / 3.0;
+      T.w[0] = T.w[1] = T.w[2] = 1.0 / 3.0;
+      return true;
+    case RGRMHD_TIME_IMEX_SSP3_332:
+      T.s = 3;
+      T.At[1][0] = 1.0; T.At[2][0] = 0.25; T.At[2][1] = 0.25; T.wt[0] = T.wt[1] = 1.0 / 6.0; T.wt[2] = 2.0 / 3.0;
+      T.A[0][0] = g; T.A[1][0] = 1.0 - 2.0 * g; T.A[1][1] = g; T.A[2][0] = 0.5 - g; T.A[2][2] = g;
+      T.w[0] = T.w[1] = 1.0 / 6.0; T.w[2] = 2.0 / 3.0;
+      return true;
+    case RGRMHD_TIME_IMEX_SSP3_433: {
+      const double al = 0.24169426078821, be = 0.06042356519705, et = 0.12915286960590;
+      T.s = 4;
+      T.At[2][1] = 1.0; T.At[3][1] = 0.25; T.At[3][2] = 0.25; T.wt[1] = T.wt[2] = 1.0 / 6.0; T.wt[3] = 2.0 / 3.0;
+      T.A[0][0] = al; T.A[1][0] = -al; T.A[1][1] = al; T.A[2][1] = 1.0 - al; T.A[2][2] = al;
+      T.A[3][0] = be; T.A[3][1] = et; T.A[3][2] = 0.5 - be - et - al; T.A[3][3] = al;
+      T.w[1] = T.w[2] = 1.0 / 6.0; T.w[3] = 2.0 / 3.0;
+      return true;
+    }
+  }
+  return false;
+}
+}  // namespace
+
+static int step_general(rgrmhd_t h, double dt, int recon, const Tableau& T) {
+  DeviceGuard guard(h->device);
+  const rg::GridView& G = h->G;
+  cudaStream_t st = h->stream;
+  const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
+  int rc;
+  if ((rc = finish_step(h))) return rc;                       // a deferred recovery of the SSP2(2,2,2) path, if any
+  if (T.s > 2 && !h->slab2) {                                 // accumulators of stages 2 and 3
+    const size_t bytes = (size_t)2 * rg::NCONS * (size_t)h->field_stride * sizeof(double);
+    if (cudaMalloc((void**)&h->slab2, bytes) != cudaSuccess) { cudaGetLastError(); h->slab2 = nullptr; return RGRMHD_E_NOMEM; }
+  }
+  rg::StageGen W;
+  std::memset(&W, 0, sizeof(W));
+  W.nstages = T.s;
+  for (int v = 0; v < rg::NCONS; ++v) {
+    W.acc[4].f[v] = G.Un[v];
+    W.acc[1].f[v] = G.Us[v];
+    W.acc[2].f[v] = h->slab2 ? h->slab2 + (size_t)v * h->field_stride : nullptr;
+    W.acc[3].f[v] = h->slab2 ? h->slab2 + (size_t)(rg::NCONS + v) * h->field_stride : nullptr;
+    W.acc[0].f[v] = G.Un[v];                                  // never used as a target
+  }
+  double* ghost_fields[rg::NPRIM + 3];
+  for (int v = 0; v < rg::NPRIM; ++v) ghost_fields[v] = G.P[v];
+  for (int q = 0; q < 3; ++q) ghost_fields[rg::NPRIM + q] = G.jc[q];
+  const int nghost_fields = rg::NPRIM + (G.charge_mode != rg::CHARGE_FACE_OHM ? 3 : 0);
+  const bool div_e = G.charge_mode == rg::CHARGE_DIV_E;
+  const bool any_active = G.n[0] > 1 || G.n[1] > 1 || G.n[2] > 1;
+  const bool tma = h->rhs_variant == 0 && h->tma != nullptr;
+  const bool pencil = !tma && h->rhs_variant != 1 && rg::rhs_pencil_supported(G);
+  h->last_rhs_variant = tma ? 0 : pencil ? 2 : 1;
+#define RG_STEP(call)                                                              \
+  do {                                                                             \
+    cudaError_t e__ = (call);                                                      \
+    if (e__ != cudaSuccess) { h->poisoned = true; h->pending_final = false; return fail_cuda(h, e__, #call); } \
+  } while (0)
+  bool have_d = false;                                        // G.dU holds dt (-div F) of the previous stage
+  for (int i = 0; i <= T.s; ++i) {
+    const bool final = i == T.s;
+    W.stage = i;
+    W.init = (i == 0);
+    W.use_dprev = have_d ? 1 : 0;
+    W.aii = final ? 0.0 : T.A[i][i];
+    for (int slot = 0; slot < 5; ++slot) {
+      const int tgt = slot == 4 ? T.s : slot;                 // row of the tableau; row s = the weights
+      auto at = [&](int row, int col) { return col < 0 ? 0.0 : row == T.s ? T.wt[col] : T.At[row][col]; };
+      auto ai = [&](int row, int col) { return row == T.s ? T.w[col] : T.A[row][col]; };
+      W.w_dprev[slot] = (have_d && tgt >= i && slot < 5 && (slot == 4 || slot < T.s)) ? at(tgt, i - 1) : 0.0;
+      W.w_src[slot] = (!final && tgt > i && (slot == 4 || slot < T.s)) ? at(tgt, i) : 0.0;
+      W.w_stiff[slot] = (!final && tgt > i && (slot == 4 || slot < T.s)) ? ai(tgt, i) / T.A[i][i] : 0.0;
+    }
+    RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_stage_gen(G, W, dt, h->stats_dev, st); }));
+    ++h->launches;
+    if (final) break;
+    bool used = T.wt[i] != 0.0;
+    for (int k = i + 1; k < T.s; ++k) used = used || T.At[k][i] != 0.0;
+    have_d = used;
+    if (!used) continue;                                      // nobody needs F of this stage (SSP3(4,3,3), stage 1)
+    if (any_active) { RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); })); ++h->launches; }
+    if (div_e) {
+      RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_div_e(G, 0, dt, st); }));
+      RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_sources_gen(G, W, dt, st); }));
+      h->launches += 2;
+    }
+    RG_STEP(timed(h, RGRMHD_K_RHS, [&] {
+      return tma    ? rg::launch_rhs_tma(G, h->tma, dt, 1, recon, h->sm_count, st)
+           : pencil ? rg::launch_rhs_pencil(G, dt, 1, recon, h->sm_count, st)
+                    : rg::launch_rhs_simple(G, dt, 1, recon, st);
+    }));                                                      // stage-1 flavour: writes dU = dt (-div F)
+    ++h->launches;
+  }
+#undef RG_STEP
+  h->pending_final = false;
+  h->charge_final_due = div_e;
+  h->solves += (T.s + 1) * nint;
+  return RGRMHD_OK;
+}
+
 int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
   if (!h || !(dt > 0.0)) return RGRMHD_E_INVALID;
   const int recon = scheme & RGRMHD_RECON_MASK;
-  if (recon > RGRMHD_RECON_WENO5 || (scheme & ~RGRMHD_RECON_MASK) != RGRMHD_TIME_IMEX_SSP2_222) return RGRMHD_E_INVALID;
+  const int time_scheme = scheme & ~RGRMHD_RECON_MASK;
+  Tableau T;
+  if (recon > RGRMHD_RECON_WENO5 || (time_scheme != RGRMHD_TIME_IMEX_SSP2_222 && !tableau_of(time_scheme, T)))
+    return RGRMHD_E_INVALID;
   if (!h->have_metric || !h->have_prims || (h->par.sigma_model == RGRMHD_SIGMA_ARRAY && !h->have_sigma) || h->poisoned)
     return RGRMHD_E_STATE;
+  if (time_scheme != RGRMHD_TIME_IMEX_SSP2_222) return step_general(h, dt, recon, T);
   DeviceGuard guard(h->device);
   const rg::GridView& G = h->G;
   cudaStream_t st = h->stream;

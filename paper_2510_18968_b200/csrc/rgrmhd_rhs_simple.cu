@@ -146,7 +146,7 @@ cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, 
 // Writes q into P and applies the two explicit source terms that carry the charge,
 //   S(calE^i) -= alpha calQ v^i,   S(Psi) += alpha calQ            (Eq. 27 / reading R1),
 // to the bracket of the next stage vector (STAGE 1: U*2 += dt ...; STAGE 2: U^{n+1} += dt/2 ...);
-// STAGE 3 (new state, on output): q and calQ = sqrt(gamma) q only.
+// STAGE 3 (new state, on output): q and calQ = sqrt(gamma) q only; STAGE 0 (general tableau driver): q only.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double sqrtg_cell(const GridView& G, long long c) {
   const double gxx = __ldg(G.met[MGXX] + c), gxy = __ldg(G.met[MGXY] + c), gxz = __ldg(G.met[MGXZ] + c);
@@ -173,7 +173,9 @@ k_charge_div_e(const __grid_constant__ GridView G, double dt) {
     }
   }
   G.P[QCH][c] = div / sqrtg_cell(G, c);
-  if (STAGE == 3) {
+  if (STAGE == 0) {
+    // general tableau driver: q only; k_charge_sources_gen distributes the source terms
+  } else if (STAGE == 3) {
     G.Un[CQ][c] = div;
   } else {
     const double w = (STAGE == 1) ? dt : 0.5 * dt, aq = __ldg(G.met[MALP] + c) * div;
@@ -188,7 +190,8 @@ cudaError_t launch_charge_div_e(const GridView& G, int stage, double dt, cudaStr
   const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
   const int threads = 128;
   const unsigned blocks = (unsigned)((nint + threads - 1) / threads);
-  if (stage == 1) k_charge_div_e<1><<<blocks, threads, 0, st>>>(G, dt);
+  if (stage == 0) k_charge_div_e<0><<<blocks, threads, 0, st>>>(G, dt);
+  else if (stage == 1) k_charge_div_e<1><<<blocks, threads, 0, st>>>(G, dt);
   else if (stage == 2) k_charge_div_e<2><<<blocks, threads, 0, st>>>(G, dt);
   else k_charge_div_e<3><<<blocks, threads, 0, st>>>(G, dt);
   return cudaGetLastError();

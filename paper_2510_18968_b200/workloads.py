@@ -52,6 +52,8 @@ SIGMA_UNIFORM, SIGMA_ARRAY, SIGMA_POWER_D, SIGMA_ATMO = 0, 1, 2, 3
 RECON_MINMOD, RECON_MC, RECON_WENO5 = 0, 1, 2
 CHARGE_FACE_OHM, CHARGE_CELL_CURRENT, CHARGE_DIV_E = 0, 1, 2
 WAVE_LIGHT, WAVE_MHD_INSIDE = 0, 1
+# time schemes: `scheme` argument of step = recon | (time << 8)
+TIME_SSP2_222, TIME_SSP2_332, TIME_SSP3_332, TIME_SSP3_433, TIME_SSP2_222_GENERAL = 0, 1 << 8, 2 << 8, 3 << 8, 4 << 8
 
 
 def splitmix64_uniform(seed: int, idx: np.ndarray) -> np.ndarray:

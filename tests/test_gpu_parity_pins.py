@@ -300,3 +300,80 @@ def test_wave_speed_mode_mhd_inside(binding, variant):
             h.step(w.dt, w.recon)
     assert np.array_equal(gl.get_prims(), goff.get_prims())
     assert not np.array_equal(gl.get_prims(), g.get_prims())
+
+
+# ----------------------------------------------------------------------------------------------
+# f2: the other IMEX-RK schemes through the general tableau driver (Eq. 32-34)
+# ----------------------------------------------------------------------------------------------
+TIME_SCHEMES = {"ssp2_332": wl.TIME_SSP2_332, "ssp3_332": wl.TIME_SSP3_332, "ssp3_433": wl.TIME_SSP3_433,
+                "ssp2_222_general": wl.TIME_SSP2_222_GENERAL}
+
+
+@pytest.mark.parametrize("name", sorted(TIME_SCHEMES))
+def test_imex_tableau_driver(binding, name):
+    """Each scheme against the oracle's literal Eq. 32 on (i) a curved periodic block (all three flux kernels),
+    (ii) a config-4 sub-block, (iii) the config-5 block across the stellar surface (floor resets with write-back in the
+    final kernel), (iv) a 1D shocktube, (v) charge mode DIV_E."""
+    from test_oracle_scheme import _pad_periodic, _periodic_problem
+    ts = TIME_SCHEMES[name]
+    rng = np.random.default_rng(41)
+    n = (38, 21, 9)
+    metric, P = _periodic_problem(40, rng, True)
+    sl = (slice(None), slice(0, n[2]), slice(0, n[1]), slice(0, n[0]))
+    metric, P = _pad_periodic(np.ascontiguousarray(metric[sl])), _pad_periodic(np.ascontiguousarray(P[sl]))
+    dt = 0.2 / 40
+    for variant in (0, 1, 2):
+        for charge in (wl.CHARGE_CELL_CURRENT, wl.CHARGE_DIV_E) if variant == 0 else (wl.CHARGE_CELL_CURRENT,):
+            par = dict(n=n, dx=(1 / 40,) * 3, bc=(0, 0, 0), gamma_eos=5 / 3, sigma_model=0, sigma0=30.0, kappa=1.0,
+                       charge_mode=charge)
+            g, o = _both(binding, par, metric, P, variant)
+            g.step(dt, wl.RECON_WENO5 | ts); o.step(dt, wl.RECON_WENO5 | ts)
+            _compare(g, o, n, 1 / 40, TOL1, "%s 1 step variant %d charge %d" % (name, variant, charge))
+            for _ in range(4):
+                g.step(dt, wl.RECON_WENO5 | ts); o.step(dt, wl.RECON_WENO5 | ts)
+            _compare(g, o, n, 1 / 40, TOL20, "%s 5 steps" % name)
+            assert g.stats()["c2p_failures"] == 0 and g.stats()["c2p_solves"] == o.stats()["c2p_solves"]
+    w = wl.blast_curved()
+    nb, bc = (40, 36, 20), (wl.BC_OUTFLOW,) * 3
+    f = w.fields((120, 138, 100), nb)
+    o = oracle.from_workload(w, fields=f, omp=True, n=nb, bc=bc)
+    g = binding.from_workload(w, fields=f, n=nb, bc=bc)
+    for _ in range(10):
+        g.step(w.dt, w.recon | ts); o.step(w.dt, w.recon | ts)
+    _compare(g, o, nb, w.dx[0], TOL20, name + " cfg4 block")
+    w = wl.tov_like()
+    i_surf = int(round((8.125 + 12.0) / w.dx[0]))
+    nb = (40, 12, 10)
+    f = w.fields((i_surf - 20, 256 - 6, 256 - 5), nb)
+    o = oracle.from_workload(w, fields=f, omp=True, n=nb, bc=bc)
+    g = binding.from_workload(w, fields=f, n=nb, bc=bc)
+    for _ in range(5):
+        g.step(w.dt, w.recon | ts); o.step(w.dt, w.recon | ts)
+    _compare(g, o, nb, w.dx[0], TOL20, name + " cfg5 block")
+    assert g.stats()["floor_resets"] == o.stats()["floor_resets"] > 0
+    w1 = wl.shocktube(n=100)
+    f1 = w1.fields()
+    o = oracle.from_workload(w1, fields=f1)
+    g = binding.from_workload(w1, fields=f1)
+    for _ in range(20):
+        g.step(w1.dt, w1.recon | ts); o.step(w1.dt, w1.recon | ts)
+    _compare(g, o, w1.n, w1.dx[0], TOL20, name + " 1D")
+
+
+def test_general_driver_reproduces_the_tuned_ssp2_222_path(binding):
+    """SSP2(2,2,2) through the general driver and through the production kernels (regrouped stage algebra, deferred
+    final recovery): same scheme, agreement to round-off; and mixing the two on one handle is allowed."""
+    w = wl.blast_curved()
+    nb, bc = (40, 36, 20), (wl.BC_OUTFLOW,) * 3
+    f = w.fields((120, 138, 100), nb)
+    ga = binding.from_workload(w, fields=f, n=nb, bc=bc)
+    gb = binding.from_workload(w, fields=f, n=nb, bc=bc)
+    gc = binding.from_workload(w, fields=f, n=nb, bc=bc)
+    for s in range(6):
+        ga.step(w.dt, w.recon)
+        gb.step(w.dt, w.recon | wl.TIME_SSP2_222_GENERAL)
+        gc.step(w.dt, w.recon | (wl.TIME_SSP2_222_GENERAL if s % 2 else wl.TIME_SSP2_222))
+    Pa, Pb, Pc = (interior(h.get_prims(), nb) for h in (ga, gb, gc))
+    sc = prim_group_scales(Pa, w.dx[0])
+    assert rel_linf(Pb, Pa, sc).max() <= 1e-13 and rel_linf(Pc, Pa, sc).max() <= 1e-13
+    assert ga.stats()["c2p_solves"] == gb.stats()["c2p_solves"] == gc.stats()["c2p_solves"]
