@@ -61,6 +61,16 @@ def roof_kernel(variant: int) -> str:
     return {0: "k_flux_tma", 1: "k_rhs_simple", 2: "k_rhs_pencil"}[variant]
 
 
+def oracle_flop_count(cfg: str):
+    """The instrumented count of the oracle's own arithmetic for one zone-cycle of `cfg` (oracle/flop_count.json,
+    written by `python -m oracle.count_flops`; a data file: nothing under oracle/ is executed here), or None."""
+    p = os.path.join(ROOT, "oracle", "flop_count.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        return json.load(f).get(cfg)
+
+
 def ncu_traffic(kernel: str, workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
     (profiles/ncu_traffic.md), or None if that kernel / workload was not captured."""
@@ -225,6 +235,71 @@ class Ranks:
 # ----------------------------------------------------------------------------------------------
 # the CUDA path
 # ----------------------------------------------------------------------------------------------
+def measure_resident(g, w, dt, steps, warmup, stream, barrier, max_over_ranks):
+    """W untimed warm-up steps, then exactly K steps between CUDA events on the launching stream (barrier +
+    synchronize on both sides); state resident in HBM; per-kernel-class device times from the library's own events."""
+    import torch
+    for _ in range(warmup):
+        g.step(dt, w.recon)
+    g.flush()                                          # the warm-up's deferred final recovery stays outside
+    g.get_timing()
+    g.reset_stats()
+    l0 = g.launch_count()
+    g.set_timing(True)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        g.step(dt, w.recon)
+    g.flush()                                          # the last step's final recovery is part of the K steps
+    e1.record(stream)
+    barrier()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    launches = g.launch_count() - l0
+    timing = g.get_timing()
+    g.set_timing(False)
+    stats = g.stats()
+    finite = bool(np.isfinite(g.get_prims()).all())
+    return {"ms_total": ms_total, "launches": launches, "timing": timing, "stats": stats, "finite": finite}
+
+
+def step_roofline(w, stats, zc_per_s_per_gpu, fp64_peak, hbm_gbs):
+    """north_star: the slower of the algorithmic bytes at HBM bandwidth and the algorithmic FP64 flops at peak."""
+    evals_per_solve = stats["c2p_evals"] / max(stats["c2p_solves"], 1)
+    ndir = sum(1 for m in w.n if m > 1)
+    step_flops = (2 * RHS_FLOPS[w.recon] * ndir / 3.0 + 2 * SRC_FLOPS + 3 * C2P_SETUP_FLOPS +
+                  3 * evals_per_solve * C2P_EVAL_FLOPS)
+    step_bytes = STEP_DOUBLES * 8.0
+    t = max(step_flops / (fp64_peak * 1e12), step_bytes / (hbm_gbs * 1e9))
+    return {"zone_cycles_per_s_at_roofline": 1.0 / t, "frac": zc_per_s_per_gpu * t, "flops_per_zone_cycle": step_flops,
+            "bytes_per_zone_cycle": step_bytes, "c2p_evals_per_solve": evals_per_solve,
+            "flop_count": "minimal-operation hand count of the scheme's formulas (DESIGN.md Sec. 7.5)"}
+
+
+EXTRA_STEPS = {"cfg1": 200, "cfg2": 200, "cfg3": 20, "cfg4": 10, "cfg5": 5}
+
+
+def measure_extra_config(binding, name, local, stream, fp64_peak, hbm_gbs):
+    """The other BASELINE configs, measured in the same run with the same code (state resident, W = 3)."""
+    w = wl.get(name)
+    g = binding.from_workload(w, device=local)
+    g.set_stream(stream.cuda_stream)
+    dt = w.cfl / g.max_speed()
+    steps = EXTRA_STEPS[name]
+    m = measure_resident(g, w, dt, steps, 3, stream, lambda: __import__("torch").cuda.synchronize(), lambda x: x)
+    ms = m["ms_total"] / steps
+    zc = w.ncells * steps / (m["ms_total"] * 1e-3)
+    out = {"n": list(w.n), "steps": steps, "ms_per_step": ms, "zone_cycles_per_s": zc,
+           "kernel_ms_per_step": {k: v[0] / steps for k, v in m["timing"].items()},
+           "gpu_launches": int(m["launches"]), "rhs_kernel": roof_kernel(g.get_rhs_variant()), "finite": m["finite"],
+           "c2p_failures": m["stats"]["c2p_failures"], "floor_resets": m["stats"]["floor_resets"]}
+    sr = step_roofline(w, m["stats"], zc, fp64_peak, hbm_gbs)
+    out["step_roofline_frac"] = sr["frac"] if w.ncells >= 1 << 20 else None     # launch-bound below: absolute numbers only
+    out["c2p_evals_per_solve"] = sr["c2p_evals_per_solve"]
+    g.close()
+    return out
+
+
 def run_ours(args):
     import torch
     from paper_2510_18968_b200 import binding
@@ -249,32 +324,14 @@ def run_ours(args):
     hbm_gbs, peak_kind = load_peaks()
 
     # ---- device-resident timing ------------------------------------------------------------------
-    for _ in range(args.warmup):
-        g.step(dt, w.recon)
-    g.flush()                                          # the warm-up's deferred final recovery stays outside
-    g.get_timing()
-    l0 = g.launch_count()
-    g.set_timing(True)
     sampler = ClockSampler(local) if rank == 0 else None
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.time()
-    e0.record(stream)
-    for _ in range(args.steps):
-        g.step(dt, w.recon)
-    g.flush()                                          # the last step's final recovery is part of the K steps
-    e1.record(stream)
-    barrier()
+    m = measure_resident(g, w, dt, args.steps, args.warmup, stream, barrier, max_over_ranks)
     t1 = time.time()
-    ms_total = max_over_ranks(e0.elapsed_time(e1))
     clocks = sampler.stop(t0, t1) if sampler else None
-    launches = g.launch_count() - l0
-    timing = g.get_timing()
-    g.set_timing(False)
-    stats = g.stats()
-    P_end = g.get_prims()
-    finite = bool(np.isfinite(P_end).all())
+    ms_total, launches, timing, stats, finite = m["ms_total"], m["launches"], m["timing"], m["stats"], m["finite"]
     value = world * w.ncells * args.steps / (ms_total * 1e-3)
+    variant_used = g.get_rhs_variant()
 
     # ---- end to end through the C-ABI with host buffers ------------------------------------------
     e2e = None
@@ -286,6 +343,7 @@ def run_ours(args):
         for _ in range(1):
             g.set_prims(pin_in); g.step(dt, w.recon); g.get_prims(pin_out)
         barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(k_e2e):
             g.set_prims(pin_in)
@@ -317,8 +375,9 @@ def run_ours(args):
         roof = {"bound": "hbm", "achieved": nbytes_alg / rhs_avg_s / 1e9, "peak": hbm_gbs, "unit": "GB/s",
                 "peak_kind": "%s copy bandwidth (MEASURED_PEAKS.json)" % peak_kind}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = ncu_traffic(roof_kernel(args.rhs_variant), w.name)
-    roof["kernel"] = roof_kernel(args.rhs_variant)
+    roof["kernel"] = roof_kernel(variant_used)          # the kernel rgrmhd_step actually launched (fallbacks included)
+    roof["traffic"] = ncu_traffic(roof["kernel"], w.name)
+    roof["traffic_source"] = "static: ncu --set full capture of this kernel on this workload (profiles/ncu_traffic.md)"
     roof["avg_launch_ms"] = rhs_avg_s * 1e3
     roof["alg_flops_per_cell"] = RHS_FLOPS[w.recon]
     roof["alg_bytes_per_cell"] = RHS_DOUBLES * 8.0
@@ -326,15 +385,40 @@ def run_ours(args):
     step_ms = ms_total / args.steps
     shares = {k: (v[0] / args.steps) / step_ms for k, v in timing.items()}
     roof["share_of_step"] = shares["rhs"]
-    # whole-step roofline (north_star: the slower of bytes at HBM bandwidth and FP64 flops at peak)
-    evals_per_solve = stats["c2p_evals"] / max(stats["c2p_solves"], 1)
-    step_flops = (2 * RHS_FLOPS[w.recon] + 2 * SRC_FLOPS + 3 * C2P_SETUP_FLOPS +
-                  3 * evals_per_solve * C2P_EVAL_FLOPS)
-    step_bytes = STEP_DOUBLES * 8.0
-    t_step_roof = max(step_flops / (fp64_peak * 1e12), step_bytes / (hbm_gbs * 1e9))
-    step_roof = {"zone_cycles_per_s_at_roofline": 1.0 / t_step_roof, "frac": value / world * t_step_roof,
-                 "flops_per_zone_cycle": step_flops, "bytes_per_zone_cycle": step_bytes,
-                 "c2p_evals_per_solve": evals_per_solve}
+    step_roof = step_roofline(w, stats, value / world, fp64_peak, hbm_gbs)
+    # the oracle's own, instrumented operation count for this config (an upper bound: the oracle recomputes freely)
+    oc = oracle_flop_count(args.config)
+    if oc is not None:
+        f_or = oc["total_flops_per_zone_cycle_recon_once"]
+        t_or = max(f_or / (fp64_peak * 1e12), STEP_DOUBLES * 8.0 / (hbm_gbs * 1e9))
+        step_roof["oracle_instrumented"] = {
+            "flops_per_zone_cycle": f_or, "flops_per_zone_cycle_as_executed": oc["total_flops_per_zone_cycle_oracle"],
+            "by_region": oc["flops_per_zone_cycle_by_region"], "frac_if_used": value / world * t_or,
+            "note": "python -m oracle.count_flops (counting scalar, FMA = 2, div = sqrt = 1, 32^3 sub-block); the oracle's "
+                    "formulas are written for legibility, so this is an upper bound of the algorithmic work and `frac` "
+                    "above keeps the smaller hand count"}
+
+    # ---- the other BASELINE configs, same run, same code ---------------------------------------------
+    configs = {args.config: {"n": list(w.n), "steps": args.steps, "ms_per_step": step_ms,
+                             "zone_cycles_per_s": value / world,
+                             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in timing.items()},
+                             "step_roofline_frac": step_roof["frac"], "rhs_kernel": roof["kernel"],
+                             "c2p_evals_per_solve": step_roof["c2p_evals_per_solve"]}}
+    if world == 1 and not args.no_extra_configs:
+        g.close()
+        del f
+        for name in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5"):
+            if name == args.config:
+                continue
+            if name == "cfg5":
+                free, _ = torch.cuda.mem_get_info()
+                if free < 135e9:
+                    configs[name] = {"skipped": "needs 126 GB of device memory, %.0f GB free" % (free / 1e9)}
+                    continue
+            try:
+                configs[name] = measure_extra_config(binding, name, local, stream, fp64_peak, hbm_gbs)
+            except Exception as e:  # a failed extra config must not lose the headline line
+                configs[name] = {"error": str(e)[:200]}
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -348,9 +432,10 @@ def run_ours(args):
                        "time": "imex_ssp2_222", "dt": dt, "parallelism": "replicas only x%d" % world,
                        "l2": "inputs larger than L2 (%.0f MB of fields per kernel vs 126 MB)" %
                              (RHS_DOUBLES * 8 * w.ncells / 1e6),
-                       "rhs_variant": args.rhs_variant},
+                       "rhs_variant": variant_used},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof,
             "step_roofline": step_roof, "kernel_ms_per_step": {k: v[0] / args.steps for k, v in timing.items()},
+            "configs": configs,
             "cpu_baseline": cpu, "finite": finite, "c2p": stats}
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -370,6 +455,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra-configs", action="store_true",
+                    help="skip the `configs` object (the other BASELINE configs measured in the same run)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                     # timing rule: W >= 3

@@ -20,7 +20,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rgrmhd_oracle.cpp")
-_LIBS: Dict[bool, C.CDLL] = {}
+_LIBS: Dict[object, C.CDLL] = {}
 
 NPRIM = NCONS = 14
 
@@ -53,13 +53,31 @@ class Stats(C.Structure):
                 ("floor_resets", C.c_longlong), ("c2p_max_evals", C.c_int), ("reserved", C.c_int)]
 
 
-def lib(omp: bool = False) -> C.CDLL:
+def build_count() -> str:
+    """The instrumented variant (-DORACLE_COUNT_FLOPS: a counting scalar replaces double; oracle/flopcount.h).  Used by
+    oracle/count_flops.py only."""
+    out = os.path.join(_HERE, "liboracle_count.so")
+    hdr = os.path.join(_HERE, "flopcount.h")
+    if not (os.path.exists(out) and os.path.getmtime(out) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
+        tmp = out + ".tmp%d" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-Wno-unknown-pragmas",
+                               "-DORACLE_COUNT_FLOPS", "-I", _HERE, "-o", tmp, _SRC])
+        os.replace(tmp, out)
+    return out
+
+
+def lib(omp=False) -> C.CDLL:
+    """omp: False (single thread: the oracle by definition), True (OpenMP build), or "count" (instrumented build)."""
     if omp not in _LIBS:
-        build()
-        if omp:   # libgomp reads these when it is first loaded; an unset thread count makes it 10x slower on small grids here
+        if omp == "count":
+            path = build_count()
+        else:
+            build()
+            path = os.path.join(_HERE, "liboracle_omp.so" if omp else "liboracle.so")
+        if omp is True:   # libgomp reads these when it is first loaded; an unset thread count makes it 10x slower on small grids here
             ncpu = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
             os.environ.setdefault("OMP_NUM_THREADS", str(ncpu))
-        L = C.CDLL(os.path.join(_HERE, "liboracle_omp.so" if omp else "liboracle.so"))
+        L = C.CDLL(path)
         L.oracle_max_speed.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.oracle_sigma_point.restype = C.c_double
@@ -67,7 +85,7 @@ def lib(omp: bool = False) -> C.CDLL:
         for name in ("oracle_prim2cons_point", "oracle_c2p_point", "oracle_c2p_literal_point", "oracle_c2p_plain_point",
                      "oracle_implicit_E_point", "oracle_state_flux_point", "oracle_recon_1d"):
             getattr(L, name).restype = C.c_int
-        if omp:   # the cores this process may run on (a container's cpu set can be smaller than the host's count)
+        if omp is True:   # the cores this process may run on (a container's cpu set can be smaller than the host's count)
             L.oracle_set_threads(len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
         _LIBS[omp] = L
     return _LIBS[omp]
@@ -105,7 +123,7 @@ def make_params(p: dict) -> Params:
 class Oracle:
     """Handle-level wrapper mirroring include/rgrmhd.h (host NumPy arrays)."""
 
-    def __init__(self, params: dict, omp: bool = False):
+    def __init__(self, params: dict, omp=False):
         self.L = lib(omp)
         self.par = make_params(params)
         self.h = C.c_void_p()
@@ -199,7 +217,7 @@ class Oracle:
         self.L.oracle_reset_stats(self.h)
 
 
-def from_workload(w, fields: Optional[dict] = None, omp: bool = False, n=None, bc=None, solver: str = "plain",
+def from_workload(w, fields: Optional[dict] = None, omp=False, n=None, bc=None, solver: str = "plain",
                   **over) -> Oracle:
     """Create an oracle handle for workload `w` (or a sub-block of it) and load its fields."""
     par = w.params(n=n, bc=bc)

@@ -35,6 +35,17 @@
 #include <omp.h>
 #endif
 
+// Instrumented build (oracle/count_flops.py): every `double` below becomes a counting scalar that
+// tallies add/mul/div/sqrt per region of the step.  Same arithmetic, same results; never used by tests or timing.
+#ifdef ORACLE_COUNT_FLOPS
+#include "flopcount.h"
+namespace flopcount { long long counts[R_COUNT][OP_COUNT]; long long calls[R_COUNT]; int region = R_OTHER; }
+#define double cdouble
+#define FLOP_REGION(r) flopcount::Scope flop_scope__(flopcount::r)
+#else
+#define FLOP_REGION(r)
+#endif
+
 namespace {
 
 enum { NPRIM = 14, NCONS = 14, NMET = 16 };
@@ -211,6 +222,7 @@ double weno5_plus(double u0, double u1, double u2, double u3, double u4, double 
 }
 void recon_cell(int scheme, double eps_w, double um2, double um1, double u0, double up1, double up2,
                 double* at_minus_half, double* at_plus_half) {
+  FLOP_REGION(R_RECON);
   if (scheme == RECON_WENO5) {
     *at_plus_half = weno5_plus(um2, um1, u0, up1, up2, eps_w);
     *at_minus_half = weno5_plus(up2, up1, u0, um1, um2, eps_w);   // mirror image
@@ -383,6 +395,7 @@ struct C2PWork {
 };
 // residual g(Z) for frozen (s, kE); returns false when v^2 >= 1 (treated as g = -infinity)
 bool c2p_residual(C2PWork& w, double Z, double* g) {
+  FLOP_REGION(R_C2P_EVAL);
   const Metric& m = *w.m;
   const double A = Z + w.r * w.B2, c = w.r * w.kE;
   const double den = A * A + c * c * w.B2;
@@ -403,6 +416,7 @@ bool c2p_residual(C2PWork& w, double Z, double* g) {
 
 C2PResult c2p_robust(const Metric& m, double Gamma, const double U[NCONS], double adt, double sigma,
                      double tol, int maxit, double P[NPRIM] /* in: guess (rho, p, v); out: primitives */) {
+  FLOP_REGION(R_C2P_SETUP);
   C2PWork w;
   w.m = &m; w.Gamma = Gamma;
   const double sg = m.sqrtg;
@@ -520,6 +534,7 @@ C2PResult c2p_robust(const Metric& m, double Gamma, const double U[NCONS], doubl
 // E is the closed form of Eq. 42 at the guess velocity.
 C2PResult c2p_plain(const Metric& m, double Gamma, const double U[NCONS], double adt, double sigma,
                     double tol, int max_outer, double P[NPRIM] /* in: guess (v); out: primitives */) {
+  FLOP_REGION(R_C2P_SETUP);
   C2PWork w;
   w.m = &m; w.Gamma = Gamma;
   const double sg = m.sqrtg;
@@ -738,6 +753,7 @@ int face_states(const Grid& G, int scheme, int d, int i, int j, int k, const Met
 }
 
 int hlle_face(const Grid& G, int scheme, int d, int i, int j, int k, double Fh[NCONS]) {
+  FLOP_REGION(R_RIEMANN);
   int o[3] = {0, 0, 0}; o[d] = 1;
   const int il = i - o[0], jl = j - o[1], kl = k - o[2];
   const long cL = G.idx(il, jl, kl), cR = G.idx(i, j, k);
@@ -786,6 +802,7 @@ inline double d4(const std::vector<double>& f, long c, long stride, double dx) {
   return (-f[c + 2 * stride] + 8.0 * f[c + stride] - 8.0 * f[c - stride] + f[c - 2 * stride]) / (12.0 * dx);
 }
 void sources_cell(const Grid& G, int i, int j, int k, double S[NCONS]) {
+  FLOP_REGION(R_SOURCES);
   const long c = G.idx(i, j, k);
   const long stride[3] = {1, (long)G.np[0], (long)G.np[0] * G.np[1]};
   Metric m; metric_at(G, c, m);
@@ -853,6 +870,7 @@ void sources_cell(const Grid& G, int i, int j, int k, double S[NCONS]) {
 
 // F[U] of Eq. 31/39-40 for every interior cell: -sum_k (F^k_{+1/2} - F^k_{-1/2})/dx^k + S
 void rhs_all(Grid& G, int scheme, std::vector<double> Fout[NCONS]) {
+  FLOP_REGION(R_DIVERGENCE);
   const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2];
   for (int v = 0; v < NCONS; ++v) std::fill(Fout[v].begin(), Fout[v].end(), 0.0);
   std::vector<double> Fh[NCONS];
@@ -898,6 +916,7 @@ void rhs_all(Grid& G, int scheme, std::vector<double> Fout[NCONS]) {
 // Floor rule: reading R9.
 // ---------------------------------------------------------------------------------------------
 void solve_all(Grid& G, std::vector<double> Ust[NCONS], double adt, std::vector<double>* Xout, bool write_back_floor) {
+  FLOP_REGION(R_C2P_SETUP);
   const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2];
   long long evals = 0, failures = 0, floors = 0; int max_evals = 0;
 #pragma omp parallel for collapse(3) schedule(static) reduction(+ : evals, failures, floors) reduction(max : max_evals)
@@ -988,6 +1007,7 @@ void final_charge(Grid& G) {
 }
 
 void step(Grid& G, double dt, int scheme) {
+  FLOP_REGION(R_COMBINE);
   const double gam = 1.0 - 1.0 / std::sqrt(2.0);
   const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2];
   // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n
@@ -1076,6 +1096,7 @@ bool tableau_of(int time_scheme, Tableau& T) {
 }
 
 void step_tableau(Grid& G, double dt, int scheme, const Tableau& T) {
+  FLOP_REGION(R_COMBINE);
   const int nx = G.par.n[0], ny = G.par.n[1], nz = G.par.n[2], s = T.s;
   std::vector<double> F[4][NCONS], R[4][3], Xst[3], Xi[3];
   for (int q = 0; q < 3; ++q) { Xst[q].assign(G.ntot, 0.0); Xi[q].assign(G.ntot, 0.0); }
@@ -1149,6 +1170,7 @@ double max_speed(const Grid& G) {
 }
 
 void cons_from_prims_all(Grid& G) {
+  FLOP_REGION(R_P2C);
   for (long c = 0; c < G.ntot; ++c) {
     Metric m; metric_at(G, c, m);
     double P[NPRIM], U[NCONS];
@@ -1414,6 +1436,21 @@ int oracle_set_threads(int n) {
   return 1;
 #endif
 }
+#ifdef ORACLE_COUNT_FLOPS
+// counters of the instrumented build: out[region][op] (add, mul, div, sqrt), calls[region]
+int oracle_flops_get(long long* out, long long* calls) {
+  for (int r = 0; r < flopcount::R_COUNT; ++r) {
+    calls[r] = flopcount::calls[r];
+    for (int o = 0; o < flopcount::OP_COUNT; ++o) out[r * flopcount::OP_COUNT + o] = flopcount::counts[r][o];
+  }
+  return flopcount::R_COUNT;
+}
+int oracle_flops_reset(void) {
+  std::memset(flopcount::counts, 0, sizeof(flopcount::counts));
+  std::memset(flopcount::calls, 0, sizeof(flopcount::calls));
+  return 0;
+}
+#endif
 int oracle_omp_enabled(void) {
 #ifdef _OPENMP
   return 1;

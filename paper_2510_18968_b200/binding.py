@@ -14,7 +14,8 @@ from typing import Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "librgrmhd.so")
+# RGRMHD_LIB: load another build of the same library (kernel-variant experiments); default: the in-tree build
+_LIB_PATH = os.environ.get("RGRMHD_LIB") or os.path.join(_HERE, "librgrmhd.so")
 _LIB: Optional[C.CDLL] = None
 
 NPRIM = NCONS = 14
