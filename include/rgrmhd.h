@@ -22,7 +22,7 @@
  *
  * Ordering: all calls enqueue on the handle's stream (default: the legacy default stream;
  * rgrmhd_set_stream changes it) and return without host synchronisation, except
- * rgrmhd_max_speed and rgrmhd_get_stats (host scalars: they synchronise the stream) and
+ * rgrmhd_max_speed and rgrmhd_get_stats (host scalars: they synchronise the stream), rgrmhd_set_metric and
  * copies from/to pageable host memory (synchronous by CUDA's rules).
  *
  * Errors: every function returns 0 on success or a negative rgrmhd_status.  No exceptions
@@ -128,7 +128,10 @@ int rgrmhd_destroy(rgrmhd_t h);
 int rgrmhd_set_stream(rgrmhd_t h, void* cuda_stream);
 
 /* Fixed 3+1 metric: lapse, shift beta^i, gamma_ij, K_ij as padded
- * fields INCLUDING ghost zones (the library never extrapolates a metric). */
+ * fields INCLUDING ghost zones (the library never extrapolates a metric).  Also computes the metric-only
+ * coefficients of the geometric sources (derivatives, G^i, tr K) and allocates one field for each of them that is
+ * not identically zero on the grid (up to 34; 9 for a static conformally flat metric without shift): this call
+ * therefore synchronises the stream once and may return RGRMHD_E_NOMEM. */
 int rgrmhd_set_metric(rgrmhd_t h, const double* alpha, const double* const beta[3],
                       const double* const gam[6], const double* const K[6]);
 
@@ -156,7 +159,9 @@ int rgrmhd_flush(rgrmhd_t h);
 
 /* max over interior cells and active directions of (alpha sqrt(gamma^kk) + |beta^k|)/dx^k
  * (Eq. 30); dt = CFL / that.  With wave_speed_mode MHD_INSIDE a cell with rho > wave_rho_switch contributes
- * max(|lambda-|, |lambda+|)/dx^k of its own state instead (needs set_prims; a per-step reduction).  Synchronises. */
+ * max(|lambda-|, |lambda+|)/dx^k of its own state instead (needs set_prims; a per-step reduction).  Synchronises;
+ * in mode LIGHT the value depends on the metric only, so calls after the first one per set_metric return the cached
+ * result of that reduction without a launch. */
 int rgrmhd_max_speed(rgrmhd_t h, double* host_out);
 
 /* Current primitives (ghost zones filled by the boundary rule) / conserved variables

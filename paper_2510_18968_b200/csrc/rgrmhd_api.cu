@@ -15,7 +15,7 @@
 namespace rg {
 cudaError_t launch_c2p(const GridView& G, int stage, double dt, StatsDev* stats, cudaStream_t st);
 cudaError_t launch_prim2cons(const GridView& G, cudaStream_t st);
-cudaError_t launch_metric_coeffs(const GridView& G, cudaStream_t st);
+cudaError_t launch_metric_coeffs(const GridView& G, bool store, cudaStream_t st);
 cudaError_t launch_rhs_simple(const GridView& G, double dt, int stage, int recon, cudaStream_t st);
 cudaError_t launch_rhs_pencil(const GridView& G, double dt, int stage, int recon, int sm_count, cudaStream_t st);
 bool rhs_pencil_supported(const GridView& G);
@@ -44,6 +44,8 @@ struct rgrmhd_s {
   int device = 0;
   cudaStream_t stream = nullptr;
   double* slab = nullptr;            // all fields, one allocation
+  double* slab_src = nullptr;        // the static source-coefficient fields that are not identically zero (set_metric)
+  int nsrc_fields = 0;
   double* slab2 = nullptr;           // accumulators of the 3rd / 4th stage of the general tableau driver (allocated on first use)
   long long field_stride = 0;        // doubles between consecutive fields (ntot rounded up to 32)
   rg::StatsDev* stats_dev = nullptr;
@@ -55,6 +57,8 @@ struct rgrmhd_s {
   bool poisoned = false;        // a launch inside rgrmhd_step failed: the state is half advanced until set_prims replaces it
   int sm_count = 148;           // multiprocessors of the device (grid sizing of the flux and reduction kernels)
   bool charge_final_due = false;   // charge mode DIV_E: q, calQ of the new state not computed yet (done on output)
+  bool maxspeed_cached = false;      // wave mode LIGHT: the reduction depends on the metric only (Eq. 30): reuse it
+  double maxspeed_value = 0.0;
   int last_rhs_variant = -1;    // flux kernel the last rgrmhd_step actually launched
   int rhs_variant = 0;               // 0 = TMA-staged (default), 1 = simple, 2 = pencil (global-memory stencils)
   void* tma = nullptr;               // tensor maps of the TMA-staged flux kernel (null: shape not supported)
@@ -169,7 +173,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   G.wave_mode = p->wave_speed_mode; G.wave_rho_switch = p->wave_rho_switch;
   G.weno_eps = p->weno_eps > 0.0 ? p->weno_eps : 1e-26;
 
-  const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3 + rg::NSRC + rg::NCONS;
+  const int nfields = rg::NMET + 1 + rg::NPRIM + 3 + rg::NCONS + rg::NCONS + 3 + rg::NCONS;   // + the static source fields: set_metric
   h->field_stride = (G.ntot + 31) / 32 * 32;
   const size_t bytes = (size_t)nfields * (size_t)h->field_stride * sizeof(double);
   cudaError_t e = cudaMalloc((void**)&h->slab, bytes);
@@ -191,7 +195,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   for (int v = 0; v < rg::NCONS; ++v) G.Un[v] = next();
   for (int v = 0; v < rg::NCONS; ++v) G.Us[v] = next();
   for (int v = 0; v < 3; ++v) G.X1[v] = next();
-  for (int v = 0; v < rg::NSRC; ++v) G.src[v] = next();
+  for (int v = 0; v < rg::NSRC; ++v) G.src[v] = nullptr;   // allocated by set_metric
   for (int v = 0; v < rg::NCONS; ++v) G.dU[v] = next();
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(h->slab); cudaFree(h->stats_dev); delete h; return RGRMHD_E_CUDA; }
@@ -208,6 +212,7 @@ int rgrmhd_destroy(rgrmhd_t h) {
     for (auto& t : h->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(h->slab);
     cudaFree(h->slab2);
+    cudaFree(h->slab_src);
     cudaFree(h->stats_dev);
     rg::tma_destroy(h->tma);
   }
@@ -326,8 +331,32 @@ int rgrmhd_set_metric(rgrmhd_t h, const double* alpha, const double* const beta[
     if ((rc = copy_in(h, h->G.met[rg::MGXX + i], gam[i]))) return rc;
     if ((rc = copy_in(h, h->G.met[rg::MKXX + i], K[i]))) return rc;
   }
-  RG_CUDA(h, rg::launch_metric_coeffs(h->G, h->stream));   // static source coefficients (rgrmhd_sources.cuh)
-  ++h->launches;
+  h->maxspeed_cached = false;
+  // static source coefficients (rgrmhd_sources.cuh): find the fields that are not identically zero, allocate those, fill them
+  RG_CUDA(h, rg::launch_metric_coeffs(h->G, false, h->stream));
+  unsigned long long mask = 0;
+  RG_CUDA(h, cudaMemcpyAsync(&mask, h->G.src_mask, sizeof(mask), cudaMemcpyDeviceToHost, h->stream));
+  RG_CUDA(h, cudaStreamSynchronize(h->stream));
+  int nsrc = 0;
+  for (int q = 0; q < rg::NSRC; ++q) nsrc += (int)((mask >> q) & 1ull);
+  if (nsrc != h->nsrc_fields || !h->slab_src) {
+    cudaFree(h->slab_src);
+    h->slab_src = nullptr; h->nsrc_fields = 0;
+    if (nsrc > 0 && cudaMalloc((void**)&h->slab_src, (size_t)nsrc * (size_t)h->field_stride * sizeof(double)) != cudaSuccess) {
+      cudaGetLastError();
+      h->have_metric = false;
+      return RGRMHD_E_NOMEM;
+    }
+    h->nsrc_fields = nsrc;
+  }
+  {
+    double* q0 = h->slab_src;
+    for (int q = 0; q < rg::NSRC; ++q) {
+      if ((mask >> q) & 1ull) { h->G.src[q] = q0; q0 += h->field_stride; } else h->G.src[q] = nullptr;
+    }
+  }
+  RG_CUDA(h, rg::launch_metric_coeffs(h->G, true, h->stream));
+  h->launches += 2;
   h->have_metric = true;
   return RGRMHD_OK;
 }
@@ -541,6 +570,7 @@ int rgrmhd_max_speed(rgrmhd_t h, double* host_out) {
   if (!h || !host_out) return RGRMHD_E_INVALID;
   if (!h->have_metric) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
+  if (h->G.wave_mode == rg::WAVE_LIGHT && h->maxspeed_cached) { *host_out = h->maxspeed_value; return RGRMHD_OK; }
   RG_CUDA(h, cudaMemsetAsync(h->maxspeed_dev, 0, sizeof(unsigned long long), h->stream));
   if (h->G.wave_mode == rg::WAVE_MHD_INSIDE && h->have_prims) {   // state dependent: needs the current primitives
     int rc;
@@ -554,6 +584,7 @@ int rgrmhd_max_speed(rgrmhd_t h, double* host_out) {
   double v;
   std::memcpy(&v, &bits, sizeof(v));
   *host_out = v;
+  if (h->G.wave_mode == rg::WAVE_LIGHT) { h->maxspeed_cached = true; h->maxspeed_value = v; }
   return RGRMHD_OK;
 }
 

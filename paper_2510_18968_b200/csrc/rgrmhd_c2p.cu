@@ -209,7 +209,11 @@ k_prim2cons(const __grid_constant__ GridView G) {
   for (int v = 0; v < NCONS; ++v) G.Un[v][c] = U[v];
 }
 
-// Static source coefficients of every interior cell (once per set_metric).
+// Static source coefficients of every interior cell (once per set_metric), in two passes: STORE = false only records
+// which of the NSRC coefficient fields (and which K_ij) are not identically zero on this grid (bit mask); the host then
+// allocates exactly those fields, and STORE = true fills them (G.src[q] is null for an all-zero field: never read,
+// never written -- zero shift, K_ij = 0 and a diagonal metric leave 15 of 40 fields in BASELINE configs 4 and 5).
+template <bool STORE>
 __global__ void __launch_bounds__(128)
 k_metric_coeffs(const __grid_constant__ GridView G, unsigned long long* __restrict__ mask) {
   const int nx = G.n[0], ny = G.n[1];
@@ -222,28 +226,38 @@ k_metric_coeffs(const __grid_constant__ GridView G, unsigned long long* __restri
     const long long c = cell_index(G, i, (int)(r % ny), (int)(r / ny));
     double out[NSRC];
     metric_coeffs_cell(G, c, out);
+    if (STORE) {
 #pragma unroll
-    for (int q = 0; q < NSRC; ++q) {
-      G.src[q][c] = out[q];
-      if (out[q] != 0.0) nz |= 1ull << q;
+      for (int q = 0; q < NSRC; ++q)
+        if (G.src[q]) G.src[q][c] = out[q];
+    } else {
+#pragma unroll
+      for (int q = 0; q < NSRC; ++q)
+        if (out[q] != 0.0) nz |= 1ull << q;
+#pragma unroll
+      for (int q = 0; q < 6; ++q)
+        if (__ldg(G.met[MKXX + q] + c) != 0.0) nz |= 1ull << (NSRC + q);
     }
-#pragma unroll
-    for (int q = 0; q < 6; ++q)
-      if (__ldg(G.met[MKXX + q] + c) != 0.0) nz |= 1ull << (NSRC + q);
   }
-  // which fields are not identically zero: warp OR, one atomic per warp
-  unsigned lo = (unsigned)nz, hi = (unsigned)(nz >> 32);
-  lo = __reduce_or_sync(0xffffffffu, lo);
-  hi = __reduce_or_sync(0xffffffffu, hi);
-  if ((threadIdx.x & 31) == 0 && (lo | hi)) atomicOr(mask, ((unsigned long long)hi << 32) | lo);
+  if (!STORE) {   // which fields are not identically zero: warp OR, one atomic per warp
+    unsigned lo = (unsigned)nz, hi = (unsigned)(nz >> 32);
+    lo = __reduce_or_sync(0xffffffffu, lo);
+    hi = __reduce_or_sync(0xffffffffu, hi);
+    if ((threadIdx.x & 31) == 0 && (lo | hi)) atomicOr(mask, ((unsigned long long)hi << 32) | lo);
+  }
 }
 
-cudaError_t launch_metric_coeffs(const GridView& G, cudaStream_t st) {
+cudaError_t launch_metric_coeffs(const GridView& G, bool store, cudaStream_t st) {
   const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
   unsigned long long* mask = const_cast<unsigned long long*>(G.src_mask);
-  cudaError_t e = cudaMemsetAsync(mask, 0, sizeof(unsigned long long), st);
-  if (e != cudaSuccess) return e;
-  k_metric_coeffs<<<(unsigned)((nint + 127) / 128), 128, 0, st>>>(G, mask);
+  const unsigned blocks = (unsigned)((nint + 127) / 128);
+  if (store) {
+    k_metric_coeffs<true><<<blocks, 128, 0, st>>>(G, mask);
+  } else {
+    cudaError_t e = cudaMemsetAsync(mask, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    k_metric_coeffs<false><<<blocks, 128, 0, st>>>(G, mask);
+  }
   return cudaGetLastError();
 }
 
