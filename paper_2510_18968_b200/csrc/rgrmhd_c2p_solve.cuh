@@ -97,13 +97,9 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
   const double Wg = rsqrt_fast(1.0 - v2g);
   double W = Wg;
   double kE = dot3(vg, Es) * W * rcp_fast(W + s0);          // (v.E*)/(1 + s/W^2), s = s0 W
-  if (!(Dh > 0.0) || !(Zhi > Zlo)) {   // no physical bracket: keep the guess, E from the guess v
-    double Eh[3], EU[3];
-    implicit_E_closed(vg, W, s0 * W, Es, B, Eh);
-    triad_to_contra(t, Eh, EU);
-    P[EX] = EU[0]; P[EY] = EU[1]; P[EZ] = EU[2];
-    return res;
-  }
+  // no physical bracket: a failure; keep the guess, E from the guess v (the tail below does exactly that for a lane
+  // without a valid state).  Such a lane must NOT leave early: the loop's warp vote names every lane that entered.
+  const bool no_bracket = !(Dh > 0.0) || !(Zhi > Zlo);
   double Z = (P[RHO] + gog1 * P[PRS]) * W * W;
   bool converged = false, state_ok = false;
   const int max_outer = 50;
@@ -118,7 +114,7 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
   double a = Zlo, b = Zhi, x = Z, f = 0, xp = 0, fp = 0;
   bool ok = false, okp = false;
   int outer = 0;
-  bool need_setup = true, done = false;
+  bool need_setup = true, done = no_bracket;
   // ONE loop, one residual evaluation per trip.
   while (true) {
     if (!done) {

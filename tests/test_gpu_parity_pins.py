@@ -377,3 +377,37 @@ def test_general_driver_reproduces_the_tuned_ssp2_222_path(binding):
     sc = prim_group_scales(Pa, w.dx[0])
     assert rel_linf(Pb, Pa, sc).max() <= 1e-13 and rel_linf(Pc, Pa, sc).max() <= 1e-13
     assert ga.stats()["c2p_solves"] == gb.stats()["c2p_solves"] == gc.stats()["c2p_solves"]
+
+
+# ----------------------------------------------------------------------------------------------
+# failure paths of the recovery
+# ----------------------------------------------------------------------------------------------
+def test_recovery_failure_paths_terminate_and_follow_the_conventions(binding):
+    """(i) Tiny iteration caps: every solve stops at the cap, is counted as failed, and the step still completes
+    (round 2 found that a lane WITHOUT a physical bracket left the solver's loop early while the warp vote still named
+    it: a deadlock as soon as one cell of a warp had D^ <= 0; such states only arise after failed solves).
+    (ii) A time step far beyond the CFL limit makes the stage vector unphysical in part of the block (no bracket):
+    both sides count the same failures and, following the same conventions (keep the guess, E from the guess
+    velocity), agree on the outcome of that one step."""
+    w = wl.blast_curved()
+    n, bc = (48, 40, 24), (wl.BC_OUTFLOW,) * 3
+    f = w.fields((100, 108, 100), n)
+    for cap in (1, 2, 3):
+        g = binding.from_workload(w, fields=f, n=n, bc=bc, c2p_max_iter=cap)
+        for _ in range(4):
+            g.step(w.dt, w.recon)
+        st = g.stats()
+        assert st["c2p_max_evals"] <= cap and st["c2p_failures"] > 0 and st["c2p_solves"] == 12 * 48 * 40 * 24
+        g.get_prims()
+    dt = 40 * w.dt
+    g = binding.from_workload(w, fields=f, n=n, bc=bc)
+    o = oracle.from_workload(w, fields=f, omp=True, n=n, bc=bc)
+    g.step(dt, w.recon); o.step(dt, w.recon)
+    sg, so = g.stats(), o.stats()
+    assert so["c2p_failures"] > 0, so
+    assert sg["c2p_failures"] == so["c2p_failures"], (sg, so)
+    Pg, Po = interior(g.get_prims(), n), interior(o.get_prims(), n)
+    assert np.isfinite(Pg).all() == np.isfinite(Po).all()
+    if np.isfinite(Po).all():
+        e = rel_linf(Pg, Po, prim_group_scales(Po, w.dx[0]))
+        assert e.max() <= 1e-8, e
