@@ -300,6 +300,47 @@ def measure_extra_config(binding, name, local, stream, fp64_peak, hbm_gbs):
     return out
 
 
+def run_slabs(args, w, ranks, rank, world, local):
+    """--slabs with N > 1: ONE copy of the workload cut into N z-slabs, one per rank, with the halo exchange of
+    paper_2510_18968_b200/slab.py after each stage: strong scaling.  Not the default: the
+    north_star fixes one GPU and replicas; this build's GPU box has one GPU, so this path is
+    exercised by the single-GPU slab tests and the gloo exchange test only."""
+    import torch
+    from paper_2510_18968_b200 import binding, slab
+    s = slab.DistSlab(binding, w, device=local, rhs_variant=args.rhs_variant)
+    dt = w.cfl / s.max_speed()
+    for _ in range(args.warmup):
+        s.step(dt, w.recon)
+    s.g.flush()
+    l0 = s.g.launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ranks.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record()
+    for _ in range(args.steps):
+        s.step(dt, w.recon)
+    s.g.flush()
+    e1.record()
+    ranks.barrier()
+    t1 = time.time()
+    ms_total = ranks.max_over_ranks(e0.elapsed_time(e1))
+    clocks = sampler.stop(t0, t1) if sampler else None
+    launches = s.g.launch_count() - l0
+    finite = bool(np.isfinite(s.interior_prims()).all())
+    if rank == 0:
+        line = {"metric": METRIC, "value": w.ncells * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": w.name, "n": list(w.n), "parallelism": "z-slabs x%d, halo exchange per stage" % world,
+                           "slab_planes": s.n[2], "halo_bytes_per_face_and_exchange": s.g.halo_doubles(2) * 8},
+                "clocks": clocks, "gpu_launches": int(launches), "finite": finite, "e2e": None, "roofline": None,
+                "cpu_baseline": None}
+        print(json.dumps(line), flush=True)
+    ranks.close()
+    return 0 if finite else 1
+
+
 def run_ours(args):
     import torch
     from paper_2510_18968_b200 import binding
@@ -315,6 +356,8 @@ def run_ours(args):
     dist = ranks.dist
 
     w = get_workload(args.config)
+    if args.slabs and world > 1:
+        return run_slabs(args, w, ranks, rank, world, local)
     f = w.fields()                                     # every replica: the same seeded workload
     g = binding.from_workload(w, fields=f, device=local)
     g.set_rhs_variant(args.rhs_variant)
@@ -455,6 +498,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--slabs", action="store_true",
+                    help="N > 1 only: cut ONE copy of the workload into N z-slabs with a halo exchange per stage "
+                         "(strong scaling) instead of N replicas")
     ap.add_argument("--no-extra-configs", action="store_true",
                     help="skip the `configs` object (the other BASELINE configs measured in the same run)")
     args = ap.parse_args()

@@ -50,7 +50,12 @@ enum rgrmhd_status {
 };
 
 /* boundary conditions ("Neumann": copy nearest interior cell; PAPER.md:359 periodic) */
-enum { RGRMHD_BC_PERIODIC = 0, RGRMHD_BC_OUTFLOW = 1 };
+enum { RGRMHD_BC_PERIODIC = 0, RGRMHD_BC_OUTFLOW = 1,
+       /* the ghost layers of this direction belong to the CALLER (the block is a slab of a larger grid, PAPER.md:169
+        * "boxes"): the library never writes them; the caller fills them through
+        * rgrmhd_halo_unpack at the two exchange points of a split step (rgrmhd_step_begin / rgrmhd_step_continue).
+        * Needs n >= 3 in that direction; not available with charge mode DIV_E or the general tableau driver. */
+       RGRMHD_BC_EXTERNAL = 2 };
 
 /* conductivity models: uniform; per-cell array (BASELINE config 4); sigma0*(D/Dref)^exp
  * (Eq. 52; D undensitised, exp a non-negative integer);
@@ -147,6 +152,21 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]);
  * HLLE + flux divergence (an increment the next recovery adds to its stage vector); twice; final recovery.  The
  * other schemes: the same kernels stage by stage (Eq. 32); the first 3-/4-stage step allocates 28 more fields. */
 int rgrmhd_step(rgrmhd_t h, double dt, int scheme);
+
+/* The same SSP2(2,2,2) step in three parts, for blocks with a RGRMHD_BC_EXTERNAL direction.  rgrmhd_step_begin
+ * enqueues the recovery of stage 1 and its ghost fill; each rgrmhd_step_continue enqueues the flux divergence of the
+ * current stage and, after the first one, the recovery + ghost fill of stage 2 (*more = 1: one more exchange and one
+ * more continue are due; *more = 0: the step is complete).  Between the parts the caller moves the halo layers:
+ * rgrmhd_halo_pack copies the three INTERIOR layers next to `side` (0 = lower, 1 = upper) of direction `dir`, over the
+ * full padded extent of the other two directions, of the 14 stage primitives and the 3 conduction-current fields into
+ * dev_buf[field][layer][plane] (rgrmhd_halo_doubles doubles, DEVICE memory); rgrmhd_halo_unpack writes such a buffer
+ * into the three GHOST layers of that side.  All on the handle's stream, no synchronisation.  Every other call that
+ * reads or replaces the state returns RGRMHD_E_STATE while a split step is in flight. */
+int rgrmhd_step_begin(rgrmhd_t h, double dt, int scheme);
+int rgrmhd_step_continue(rgrmhd_t h, int* more);
+int rgrmhd_halo_doubles(rgrmhd_t h, int dir, long long* host_out);
+int rgrmhd_halo_pack(rgrmhd_t h, int dir, int side, double* dev_buf);
+int rgrmhd_halo_unpack(rgrmhd_t h, int dir, int side, const double* dev_buf);
 
 /* rgrmhd_step enqueues everything of its step except the final recovery P^{n+1} = recovery(U^{n+1}) (Eq. 37,
  * PAPER.md:209, 242).  That launch is deferred: the next rgrmhd_step runs it inside its first recovery kernel

@@ -23,7 +23,8 @@ NMETRIC = 16
 
 SYMBOLS = ["rgrmhd_params_default", "rgrmhd_create", "rgrmhd_destroy", "rgrmhd_set_stream", "rgrmhd_set_metric",
            "rgrmhd_set_sigma", "rgrmhd_set_prims", "rgrmhd_step", "rgrmhd_max_speed", "rgrmhd_get_prims",
-           "rgrmhd_get_cons", "rgrmhd_get_stats", "rgrmhd_reset_stats", "rgrmhd_set_rhs_variant", "rgrmhd_get_rhs_variant",
+           "rgrmhd_get_cons", "rgrmhd_get_stats", "rgrmhd_reset_stats", "rgrmhd_set_rhs_variant", "rgrmhd_get_rhs_variant", "rgrmhd_step_begin", "rgrmhd_step_continue", "rgrmhd_halo_doubles",
+           "rgrmhd_halo_pack", "rgrmhd_halo_unpack",
            "rgrmhd_launch_count", "rgrmhd_flush", "rgrmhd_set_timing", "rgrmhd_get_timing", "rgrmhd_measure_fp64_peak",
            "rgrmhd_strerror", "rgrmhd_last_cuda_error"]
 
@@ -75,6 +76,11 @@ def load() -> C.CDLL:
         L.rgrmhd_flush.argtypes = [vp]
         L.rgrmhd_set_rhs_variant.argtypes = [vp, C.c_int]
         L.rgrmhd_get_rhs_variant.argtypes = [vp, C.POINTER(C.c_int)]
+        L.rgrmhd_step_begin.argtypes = [vp, C.c_double, C.c_int]
+        L.rgrmhd_step_continue.argtypes = [vp, C.POINTER(C.c_int)]
+        L.rgrmhd_halo_doubles.argtypes = [vp, C.c_int, C.POINTER(C.c_longlong)]
+        L.rgrmhd_halo_pack.argtypes = [vp, C.c_int, C.c_int, vp]
+        L.rgrmhd_halo_unpack.argtypes = [vp, C.c_int, C.c_int, vp]
         L.rgrmhd_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.rgrmhd_set_timing.argtypes = [vp, C.c_int]
         L.rgrmhd_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
@@ -218,6 +224,26 @@ class Rgrmhd:
 
     def set_rhs_variant(self, variant: int):
         self._check(self.L.rgrmhd_set_rhs_variant(self.h, int(variant)), "rgrmhd_set_rhs_variant")
+
+    def step_begin(self, dt: float, scheme: int):
+        self._check(self.L.rgrmhd_step_begin(self.h, C.c_double(dt), int(scheme)), "rgrmhd_step_begin")
+
+    def step_continue(self) -> bool:
+        """Runs the next part; True if one more exchange + continue are due."""
+        more = C.c_int()
+        self._check(self.L.rgrmhd_step_continue(self.h, C.byref(more)), "rgrmhd_step_continue")
+        return bool(more.value)
+
+    def halo_doubles(self, direction: int) -> int:
+        out = C.c_longlong()
+        self._check(self.L.rgrmhd_halo_doubles(self.h, int(direction), C.byref(out)), "rgrmhd_halo_doubles")
+        return out.value
+
+    def halo_pack(self, direction: int, side: int, buf):
+        self._check(self.L.rgrmhd_halo_pack(self.h, int(direction), int(side), C.c_void_p(_ptr(buf))), "rgrmhd_halo_pack")
+
+    def halo_unpack(self, direction: int, side: int, buf):
+        self._check(self.L.rgrmhd_halo_unpack(self.h, int(direction), int(side), C.c_void_p(_ptr(buf))), "rgrmhd_halo_unpack")
 
     def get_rhs_variant(self) -> int:
         out = C.c_int()

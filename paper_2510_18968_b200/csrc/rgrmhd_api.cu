@@ -23,6 +23,8 @@ cudaError_t launch_rhs_tma(const GridView& G, const void* state, double dt, int 
 void* tma_create(const GridView& G);
 void tma_destroy(void* state);
 cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, cudaStream_t st);
+cudaError_t launch_halo_copy(const GridView& G, double* const* fields, int nf, int dir, int side, double* buf, bool pack,
+                             cudaStream_t st);
 cudaError_t launch_charge_div_e(const GridView& G, int stage, double dt, cudaStream_t st);
 cudaError_t launch_max_speed(const GridView& G, unsigned long long* out, bool have_prims, int sm_count, cudaStream_t st);
 }  // namespace rg
@@ -57,6 +59,8 @@ struct rgrmhd_s {
   bool poisoned = false;        // a launch inside rgrmhd_step failed: the state is half advanced until set_prims replaces it
   int sm_count = 148;           // multiprocessors of the device (grid sizing of the flux and reduction kernels)
   bool charge_final_due = false;   // charge mode DIV_E: q, calQ of the new state not computed yet (done on output)
+  int part = 0;                      // split step in flight: the part rgrmhd_step_continue runs next (0: none)
+  double cur_dt = 0.0; int cur_recon = 0;
   bool maxspeed_cached = false;      // wave mode LIGHT: the reduction depends on the metric only (Eq. 30): reuse it
   double maxspeed_value = 0.0;
   int last_rhs_variant = -1;    // flux kernel the last rgrmhd_step actually launched
@@ -120,7 +124,8 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
     if (p->n[d] < 1) return RGRMHD_E_INVALID;
     if (p->n[d] > 1 && !(p->dx[d] > 0.0)) return RGRMHD_E_INVALID;
     if (p->n[d] > 1 && p->n[d] < 3) return RGRMHD_E_INVALID;   // periodic wrap of 3 ghosts needs >= 3 cells
-    if (p->bc[d] != RGRMHD_BC_PERIODIC && p->bc[d] != RGRMHD_BC_OUTFLOW) return RGRMHD_E_INVALID;
+    if (p->bc[d] != RGRMHD_BC_PERIODIC && p->bc[d] != RGRMHD_BC_OUTFLOW && p->bc[d] != RGRMHD_BC_EXTERNAL) return RGRMHD_E_INVALID;
+    if (p->bc[d] == RGRMHD_BC_EXTERNAL && (p->n[d] < 3 || p->charge_mode == RGRMHD_CHARGE_DIV_E)) return RGRMHD_E_INVALID;
   }
   if (p->sigma_model < RGRMHD_SIGMA_UNIFORM || p->sigma_model > RGRMHD_SIGMA_ATMO) return RGRMHD_E_INVALID;
   if (p->charge_mode != RGRMHD_CHARGE_FACE_OHM && p->charge_mode != RGRMHD_CHARGE_CELL_CURRENT &&
@@ -245,7 +250,7 @@ static cudaError_t timed(rgrmhd_t h, int cls, const std::function<cudaError_t()>
 // runs it inside its first recovery kernel (k_c2p<4>), every other entry point that reads or replaces the state
 // launches it here first.
 static int finish_step(rgrmhd_t h) {
-  if (h->poisoned) return RGRMHD_E_STATE;
+  if (h->poisoned || h->part != 0) return RGRMHD_E_STATE;   // (a split step must be completed first)
   if (!h->pending_final) return RGRMHD_OK;
   DeviceGuard guard(h->device);
   const cudaError_t e = timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(h->G, 3, 0.0, h->stats_dev, h->stream); });
@@ -378,7 +383,8 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]) {
   if (!h->have_metric) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   int rc;
-  if (h->poisoned) { h->poisoned = false; h->pending_final = false; }   // the half-advanced state is replaced below
+  if (h->poisoned) { h->poisoned = false; h->pending_final = false; }
+  h->part = 0;   // the half-advanced state is replaced below
   if ((rc = finish_step(h))) return rc;   // keeps the statistics complete; the state itself is replaced
   for (int v = 0; v < rg::NPRIM; ++v) if ((rc = copy_in(h, h->G.P[v], prims[v]))) return rc;
   for (int q = 0; q < 3; ++q)
@@ -508,19 +514,16 @@ static int step_general(rgrmhd_t h, double dt, int recon, const Tableau& T) {
   return RGRMHD_OK;
 }
 
-int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
-  if (!h || !(dt > 0.0)) return RGRMHD_E_INVALID;
-  const int recon = scheme & RGRMHD_RECON_MASK;
-  const int time_scheme = scheme & ~RGRMHD_RECON_MASK;
-  Tableau T;
-  if (recon > RGRMHD_RECON_WENO5 || (time_scheme != RGRMHD_TIME_IMEX_SSP2_222 && !tableau_of(time_scheme, T)))
-    return RGRMHD_E_INVALID;
-  if (!h->have_metric || !h->have_prims || (h->par.sigma_model == RGRMHD_SIGMA_ARRAY && !h->have_sigma) || h->poisoned)
-    return RGRMHD_E_STATE;
-  if (time_scheme != RGRMHD_TIME_IMEX_SSP2_222) return step_general(h, dt, recon, T);
+// One IMEX-SSP2(2,2,2) step in three parts (Eq. 35-37); rgrmhd_step runs them back to back.
+//   part 0: recovery of stage 1 (+ the pending final recovery of the previous step) and its ghost fill
+//   part 1: flux divergence of stage 1, recovery of stage 2 and its ghost fill
+//   part 2: flux divergence of stage 2 (the final recovery stays deferred, see finish_step)
+static int step222_part(rgrmhd_t h, int part) {
   DeviceGuard guard(h->device);
   const rg::GridView& G = h->G;
   cudaStream_t st = h->stream;
+  const double dt = h->cur_dt;
+  const int recon = h->cur_recon;
   const long long nint = (long long)G.n[0] * G.n[1] * G.n[2];
   double* ghost_fields[rg::NPRIM + 3];
   for (int v = 0; v < rg::NPRIM; ++v) ghost_fields[v] = G.P[v];
@@ -535,35 +538,115 @@ int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
          : pencil ? rg::launch_rhs_pencil(G, dt, stage, recon, h->sm_count, st)
                   : rg::launch_rhs_simple(G, dt, stage, recon, st);
   };
-  // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n.  The recovery kernel also applies the point-wise half of the
-  // right-hand side (sources, implicit terms) to the stage target; the flux kernel adds -w dt div F.
-  // (if the previous step's final recovery is still due, the same kernel runs it first: k_c2p<4>)
-  const int first = h->pending_final ? 4 : 1;
   h->last_rhs_variant = tma ? 0 : pencil ? 2 : 1;
   // From the first launch on the state is in flight: if any launch fails, the handle is marked poisoned and every
   // later call but set_prims / destroy returns RGRMHD_E_STATE (the state is half advanced, nothing can read it safely).
 #define RG_STEP(call)                                                              \
   do {                                                                             \
     cudaError_t e__ = (call);                                                      \
-    if (e__ != cudaSuccess) { h->poisoned = true; h->pending_final = false; return fail_cuda(h, e__, #call); } \
+    if (e__ != cudaSuccess) { h->poisoned = true; h->pending_final = false; h->part = 0; return fail_cuda(h, e__, #call); } \
   } while (0)
-  RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, first, dt, h->stats_dev, st); }));
-  h->pending_final = false;
-  if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
-  if (div_e) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_div_e(G, 1, dt, st); }));
-  RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
-  // stage 2 (Eq. 36)
-  RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
-  if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
-  if (div_e) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_div_e(G, 2, dt, st); }));
-  RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
+  if (part == 0) {
+    // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n.  The recovery kernel also applies the point-wise half of the
+    // right-hand side (sources, implicit terms) to the stage target; the flux kernel adds -w dt div F.
+    // (if the previous step's final recovery is still due, the same kernel runs it first: k_c2p<4>)
+    const int first = h->pending_final ? 4 : 1;
+    RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, first, dt, h->stats_dev, st); }));
+    h->pending_final = false;
+    if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+    h->launches += 1 + (any_active ? 1 : 0);
+  } else if (part == 1) {
+    if (div_e) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_div_e(G, 1, dt, st); }));
+    RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(1); }));   // -> U*2 (Eq. 36)
+    // stage 2 (Eq. 36)
+    RG_STEP(timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(G, 2, dt, h->stats_dev, st); }));
+    if (any_active) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_ghost_fill(G, ghost_fields, nghost_fields, st); }));
+    h->launches += 2 + (any_active ? 1 : 0) + (div_e ? 1 : 0);
+  } else {
+    if (div_e) RG_STEP(timed(h, RGRMHD_K_GHOST, [&] { return rg::launch_charge_div_e(G, 2, dt, st); }));
+    RG_STEP(timed(h, RGRMHD_K_RHS, [&] { return rhs(2); }));   // -> U^{n+1} (Eq. 37)
+    // recovery of the new state at fixed calE (reading R12): deferred, see finish_step
+    h->pending_final = true;
+    h->charge_final_due = div_e;
+    h->solves += 3 * nint;
+    h->launches += 1 + (div_e ? 1 : 0);
+  }
 #undef RG_STEP
-  // recovery of the new state at fixed calE (reading R12): deferred, see finish_step
-  h->pending_final = true;
-  h->charge_final_due = div_e;
-  h->solves += 3 * nint;
-  h->launches += 4 + (any_active ? 2 : 0) + (div_e ? 2 : 0);
   return RGRMHD_OK;
+}
+
+int rgrmhd_step(rgrmhd_t h, double dt, int scheme) {
+  if (!h || !(dt > 0.0)) return RGRMHD_E_INVALID;
+  const int recon = scheme & RGRMHD_RECON_MASK;
+  const int time_scheme = scheme & ~RGRMHD_RECON_MASK;
+  Tableau T;
+  if (recon > RGRMHD_RECON_WENO5 || (time_scheme != RGRMHD_TIME_IMEX_SSP2_222 && !tableau_of(time_scheme, T)))
+    return RGRMHD_E_INVALID;
+  if (!h->have_metric || !h->have_prims || (h->par.sigma_model == RGRMHD_SIGMA_ARRAY && !h->have_sigma) || h->poisoned)
+    return RGRMHD_E_STATE;
+  if (time_scheme != RGRMHD_TIME_IMEX_SSP2_222) {
+    for (int d = 0; d < 3; ++d) if (h->G.bc[d] == rg::BC_EXTERNAL) return RGRMHD_E_INVALID;   // no exchange points inside
+    return step_general(h, dt, recon, T);
+  }
+  if (h->part != 0) return RGRMHD_E_STATE;               // a split step (rgrmhd_step_begin) is in flight
+  for (int d = 0; d < 3; ++d) if (h->G.bc[d] == rg::BC_EXTERNAL) return RGRMHD_E_INVALID;     // needs the split form
+  h->cur_dt = dt; h->cur_recon = recon;
+  int rc;
+  for (int part = 0; part < 3; ++part) if ((rc = step222_part(h, part))) return rc;
+  return RGRMHD_OK;
+}
+
+// ---- the same step in three parts, for callers that own ghost layers (bc = RGRMHD_BC_EXTERNAL: a slab of a larger
+// grid): after rgrmhd_step_begin and after the first rgrmhd_step_continue the stage's
+// primitives and conduction current are complete in the interior and in the ghost layers the library fills itself;
+// the caller exchanges the external layers (rgrmhd_halo_pack / rgrmhd_halo_unpack) and continues.
+int rgrmhd_step_begin(rgrmhd_t h, double dt, int scheme) {
+  if (!h || !(dt > 0.0)) return RGRMHD_E_INVALID;
+  const int recon = scheme & RGRMHD_RECON_MASK;
+  if (recon > RGRMHD_RECON_WENO5 || (scheme & ~RGRMHD_RECON_MASK) != RGRMHD_TIME_IMEX_SSP2_222) return RGRMHD_E_INVALID;
+  if (!h->have_metric || !h->have_prims || (h->par.sigma_model == RGRMHD_SIGMA_ARRAY && !h->have_sigma) || h->poisoned ||
+      h->part != 0)
+    return RGRMHD_E_STATE;
+  h->cur_dt = dt; h->cur_recon = recon;
+  const int rc = step222_part(h, 0);
+  if (rc == RGRMHD_OK) h->part = 1;
+  return rc;
+}
+
+int rgrmhd_step_continue(rgrmhd_t h, int* more) {
+  if (!h || !more) return RGRMHD_E_INVALID;
+  if (h->part != 1 && h->part != 2) return RGRMHD_E_STATE;
+  if (h->poisoned) return RGRMHD_E_STATE;
+  const int rc = step222_part(h, h->part);
+  if (rc != RGRMHD_OK) { h->part = 0; return rc; }
+  h->part = (h->part == 1) ? 2 : 0;
+  *more = h->part != 0;
+  return RGRMHD_OK;
+}
+
+// ---- halo layers of the stage primitives and of the conduction current (17 fields), SURVEY.md Sec. 8(e) ------------
+int rgrmhd_halo_doubles(rgrmhd_t h, int dir, long long* host_out) {
+  if (!h || !host_out || dir < 0 || dir > 2 || h->G.n[dir] < 3) return RGRMHD_E_INVALID;
+  long long plane = 1;
+  for (int d = 0; d < 3; ++d) if (d != dir) plane *= h->G.np[d];
+  *host_out = (long long)(rg::NPRIM + 3) * 3 * plane;
+  return RGRMHD_OK;
+}
+
+static int halo_copy(rgrmhd_t h, int dir, int side, double* buf, bool pack) {
+  if (!h || !buf || dir < 0 || dir > 2 || (side != 0 && side != 1) || h->G.n[dir] < 3) return RGRMHD_E_INVALID;
+  if (!h->have_prims || h->poisoned) return RGRMHD_E_STATE;
+  DeviceGuard guard(h->device);
+  double* fields[rg::NPRIM + 3];
+  for (int v = 0; v < rg::NPRIM; ++v) fields[v] = h->G.P[v];
+  for (int q = 0; q < 3; ++q) fields[rg::NPRIM + q] = h->G.jc[q];
+  RG_CUDA(h, rg::launch_halo_copy(h->G, fields, rg::NPRIM + 3, dir, side, buf, pack, h->stream));
+  ++h->launches;
+  return RGRMHD_OK;
+}
+int rgrmhd_halo_pack(rgrmhd_t h, int dir, int side, double* dev_buf) { return halo_copy(h, dir, side, dev_buf, true); }
+int rgrmhd_halo_unpack(rgrmhd_t h, int dir, int side, const double* dev_buf) {
+  return halo_copy(h, dir, side, const_cast<double*>(dev_buf), false);
 }
 
 int rgrmhd_max_speed(rgrmhd_t h, double* host_out) {

@@ -83,6 +83,7 @@ struct GhostArgs {
 __device__ __forceinline__ int ghost_src(int a, int n, int bc) {
   // a = interior-relative coordinate in [-3, n+3)
   if (a >= 0 && a < n) return a;
+  if (bc == BC_EXTERNAL) return a;                 // ghost layers owned by the caller (halo exchange): identity
   if (bc == BC_PERIODIC) return a < 0 ? a + n : a - n;
   return a < 0 ? 0 : n - 1;
 }
@@ -123,6 +124,7 @@ k_ghost_fill(const __grid_constant__ GridView G, const __grid_constant__ GhostAr
   const int sk = ghost_src(pk - G.g[2], G.n[2], G.bc[2]) + G.g[2];
   const long long dst = pi + G.stride[1] * pj + G.stride[2] * pk;
   const long long src = si + G.stride[1] * sj + G.stride[2] * sk;
+  if (dst == src) return;                          // every ghost coordinate of this cell is the caller's
   for (int v = 0; v < A.nf; ++v) A.f[v][dst] = A.f[v][src];
 }
 
@@ -137,6 +139,44 @@ cudaError_t launch_ghost_fill(const GridView& G, double* const* fields, int nf, 
   if (tot == 0) return cudaSuccess;
   const int threads = 256;
   k_ghost_fill<<<(unsigned)((tot + threads - 1) / threads), threads, 0, st>>>(G, A, gx, gy, gz);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Halo layers for a caller that owns the ghost zones of a direction (bc = BC_EXTERNAL): pack =
+// the three interior layers next to `side` of direction `dir`, over the FULL padded extent of the other two directions
+// (so that a neighbour receives the ghost columns this block has just filled in those directions: the result equals
+// the single-block fill x, then y, then z), into buf[field][layer][plane]; unpack = buf into the three ghost layers.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_halo_copy(const __grid_constant__ GridView G, const __grid_constant__ GhostArgs A, int dir, int side, double* __restrict__ buf,
+            int pack, long long plane) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= 3 * plane) return;
+  const int layer = (int)(t / plane);
+  const long long r = t % plane;
+  const int d1 = (dir == 0) ? 1 : 0, d2 = (dir == 2) ? 1 : 2;          // the other two directions, d1 faster
+  int p[3];
+  p[d1] = (int)(r % G.np[d1]);
+  p[d2] = (int)(r / G.np[d1]);
+  // padded coordinate of the layer: interior layers [g, g+3) or [g+n-3, g+n) for pack; ghost layers [0, 3) or [g+n, g+n+3) for unpack
+  const int g = G.g[dir], n = G.n[dir];
+  p[dir] = pack ? (side == 0 ? g + layer : g + n - 3 + layer) : (side == 0 ? layer : g + n + layer);
+  const long long c = p[0] + G.stride[1] * p[1] + G.stride[2] * p[2];
+  for (int v = 0; v < A.nf; ++v) {
+    double* b = buf + ((long long)v * 3 + layer) * plane + r;
+    if (pack) *b = A.f[v][c]; else A.f[v][c] = *b;
+  }
+}
+
+cudaError_t launch_halo_copy(const GridView& G, double* const* fields, int nf, int dir, int side, double* buf, bool pack,
+                             cudaStream_t st) {
+  GhostArgs A;
+  A.nf = nf;
+  for (int v = 0; v < nf; ++v) A.f[v] = fields[v];
+  long long plane = 1;
+  for (int d = 0; d < 3; ++d) if (d != dir) plane *= G.np[d];
+  k_halo_copy<<<(unsigned)((3 * plane + 255) / 256), 256, 0, st>>>(G, A, dir, side, buf, pack ? 1 : 0, plane);
   return cudaGetLastError();
 }
 

@@ -47,7 +47,7 @@ NPRIM, NCONS, NMETRIC = 14, 14, 16
 (RHO, PRS, VX, VY, VZ, EX, EY, EZ, BX, BY, BZ, PSI, PHI, QCH) = range(14)
 
 # enums mirrored from include/rgrmhd.h (plain integers, no arithmetic)
-BC_PERIODIC, BC_OUTFLOW = 0, 1
+BC_PERIODIC, BC_OUTFLOW, BC_EXTERNAL = 0, 1, 2
 SIGMA_UNIFORM, SIGMA_ARRAY, SIGMA_POWER_D, SIGMA_ATMO = 0, 1, 2, 3
 RECON_MINMOD, RECON_MC, RECON_WENO5 = 0, 1, 2
 CHARGE_FACE_OHM, CHARGE_CELL_CURRENT, CHARGE_DIV_E = 0, 1, 2
