@@ -411,3 +411,32 @@ def test_recovery_failure_paths_terminate_and_follow_the_conventions(binding):
     if np.isfinite(Po).all():
         e = rel_linf(Pg, Po, prim_group_scales(Po, w.dx[0]))
         assert e.max() <= 1e-8, e
+
+
+def test_set_metric_twice_reallocates_the_static_source_fields(binding):
+    """set_metric sizes the slab of static source coefficients by the fields that are not identically zero on the
+    grid (none in flat space, 15 for a conformally flat metric, all 34 with shift and K_ij).  Replacing the metric on a
+    live handle must give the same results as a fresh handle."""
+    from test_oracle_scheme import _pad_periodic, _periodic_problem
+    rng = np.random.default_rng(3)
+    n = (20, 18, 6)
+    metric, P = _periodic_problem(24, rng, True)
+    sl = (slice(None), slice(0, n[2]), slice(0, n[1]), slice(0, n[0]))
+    metric, P = _pad_periodic(np.ascontiguousarray(metric[sl])), _pad_periodic(np.ascontiguousarray(P[sl]))
+    flat = np.zeros_like(metric); flat[0] = 1; flat[4] = flat[7] = flat[9] = 1
+    par = dict(n=n, dx=(1 / 24,) * 3, bc=(0, 0, 0), gamma_eos=5 / 3, sigma0=20.0)
+    fresh = binding.Rgrmhd(par)
+    fresh.set_metric(metric); fresh.set_prims(P)
+    reused = binding.Rgrmhd(par)
+    reused.set_metric(flat); reused.set_prims(P)
+    reused.step(0.005, wl.RECON_WENO5)                   # flat space: no source field allocated
+    reused.set_metric(metric); reused.set_prims(P)       # now all of them
+    for h in (fresh, reused):
+        for _ in range(3):
+            h.step(0.005, wl.RECON_WENO5)
+    assert np.array_equal(fresh.get_prims(), reused.get_prims())
+    reused.set_metric(flat); reused.set_prims(P)         # and back
+    ref = binding.Rgrmhd(par)
+    ref.set_metric(flat); ref.set_prims(P)
+    reused.step(0.005, wl.RECON_WENO5); ref.step(0.005, wl.RECON_WENO5)
+    assert np.array_equal(ref.get_prims(), reused.get_prims())
