@@ -61,6 +61,7 @@ struct rgrmhd_s {
   bool charge_final_due = false;   // charge mode DIV_E: q, calQ of the new state not computed yet (done on output)
   int part = 0;                      // split step in flight: the part rgrmhd_step_continue runs next (0: none)
   double cur_dt = 0.0; int cur_recon = 0;
+  bool maxspeed_fused = false;       // wave mode MHD_INSIDE: the word holds the reduction over the CURRENT state (final recovery)
   bool maxspeed_cached = false;      // wave mode LIGHT: the reduction depends on the metric only (Eq. 30): reuse it
   double maxspeed_value = 0.0;
   int last_rhs_variant = -1;    // flux kernel the last rgrmhd_step actually launched
@@ -191,6 +192,7 @@ int rgrmhd_create(rgrmhd_t* out, const rgrmhd_params* p) {
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device);
   if (e != cudaSuccess) { cudaGetLastError(); cudaFree(h->slab); cudaFree(h->stats_dev); delete h; return RGRMHD_E_CUDA; }
   G.src_mask = h->maxspeed_dev + 1;
+  G.maxspeed_word = h->maxspeed_dev;
   double* q = h->slab;
   auto next = [&]() { double* r = q; q += h->field_stride; return r; };
   for (int v = 0; v < rg::NMET; ++v) G.met[v] = next();
@@ -253,10 +255,13 @@ static int finish_step(rgrmhd_t h) {
   if (h->poisoned || h->part != 0) return RGRMHD_E_STATE;   // (a split step must be completed first)
   if (!h->pending_final) return RGRMHD_OK;
   DeviceGuard guard(h->device);
+  const bool fuse_cfl = h->G.wave_mode == rg::WAVE_MHD_INSIDE;
+  if (fuse_cfl) RG_CUDA(h, cudaMemsetAsync(h->maxspeed_dev, 0, sizeof(unsigned long long), h->stream));
   const cudaError_t e = timed(h, RGRMHD_K_C2P, [&] { return rg::launch_c2p(h->G, 3, 0.0, h->stats_dev, h->stream); });
   if (e != cudaSuccess) { h->poisoned = true; return fail_cuda(h, e, "launch_c2p(final recovery)"); }
   ++h->launches;
   h->pending_final = false;
+  h->maxspeed_fused = fuse_cfl;
   return RGRMHD_OK;
 }
 
@@ -336,7 +341,7 @@ int rgrmhd_set_metric(rgrmhd_t h, const double* alpha, const double* const beta[
     if ((rc = copy_in(h, h->G.met[rg::MGXX + i], gam[i]))) return rc;
     if ((rc = copy_in(h, h->G.met[rg::MKXX + i], K[i]))) return rc;
   }
-  h->maxspeed_cached = false;
+  h->maxspeed_cached = false; h->maxspeed_fused = false;
   // static source coefficients (rgrmhd_sources.cuh): find the fields that are not identically zero, allocate those, fill them
   RG_CUDA(h, rg::launch_metric_coeffs(h->G, false, h->stream));
   unsigned long long mask = 0;
@@ -393,6 +398,7 @@ int rgrmhd_set_prims(rgrmhd_t h, const double* const prims[14]) {
   ++h->launches;
   h->have_prims = true;
   h->charge_final_due = false;
+  h->maxspeed_fused = false;
   return RGRMHD_OK;
 }
 
@@ -472,6 +478,7 @@ static int step_general(rgrmhd_t h, double dt, int recon, const Tableau& T) {
     cudaError_t e__ = (call);                                                      \
     if (e__ != cudaSuccess) { h->poisoned = true; h->pending_final = false; return fail_cuda(h, e__, #call); } \
   } while (0)
+  h->maxspeed_fused = false;
   bool have_d = false;                                        // G.dU holds dt (-div F) of the previous stage
   for (int i = 0; i <= T.s; ++i) {
     const bool final = i == T.s;
@@ -546,6 +553,7 @@ static int step222_part(rgrmhd_t h, int part) {
     cudaError_t e__ = (call);                                                      \
     if (e__ != cudaSuccess) { h->poisoned = true; h->pending_final = false; h->part = 0; return fail_cuda(h, e__, #call); } \
   } while (0)
+  h->maxspeed_fused = false;
   if (part == 0) {
     // stage 1 (Eq. 35): X*1 = X^n, Y1 = Y^n.  The recovery kernel also applies the point-wise half of the
     // right-hand side (sources, implicit terms) to the stage target; the flux kernel adds -w dt div F.
@@ -654,13 +662,15 @@ int rgrmhd_max_speed(rgrmhd_t h, double* host_out) {
   if (!h->have_metric) return RGRMHD_E_STATE;
   DeviceGuard guard(h->device);
   if (h->G.wave_mode == rg::WAVE_LIGHT && h->maxspeed_cached) { *host_out = h->maxspeed_value; return RGRMHD_OK; }
-  RG_CUDA(h, cudaMemsetAsync(h->maxspeed_dev, 0, sizeof(unsigned long long), h->stream));
   if (h->G.wave_mode == rg::WAVE_MHD_INSIDE && h->have_prims) {   // state dependent: needs the current primitives
     int rc;
     if ((rc = finish_step(h))) return rc;
   }
-  RG_CUDA(h, rg::launch_max_speed(h->G, h->maxspeed_dev, h->have_prims, h->sm_count, h->stream));
-  ++h->launches;
+  if (!(h->G.wave_mode == rg::WAVE_MHD_INSIDE && h->maxspeed_fused)) {   // else: the final recovery has just reduced it
+    RG_CUDA(h, cudaMemsetAsync(h->maxspeed_dev, 0, sizeof(unsigned long long), h->stream));
+    RG_CUDA(h, rg::launch_max_speed(h->G, h->maxspeed_dev, h->have_prims, h->sm_count, h->stream));
+    ++h->launches;
+  }
   unsigned long long bits = 0;
   RG_CUDA(h, cudaMemcpyAsync(&bits, h->maxspeed_dev, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
   RG_CUDA(h, cudaStreamSynchronize(h->stream));

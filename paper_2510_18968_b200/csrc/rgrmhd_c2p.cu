@@ -38,6 +38,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
   const double adt = (STAGE == 3) ? 0.0 : gam * dt;
   double* const* Ust = (STAGE == 2) ? G.Us : G.Un;
   int evals = 0, evmax = 0, failed = 0, floored = 0;
+  double cfl = 0.0;
   const bool in_range = i < G.n[0] && j < G.n[1];
   const unsigned lanes = __ballot_sync(0xffffffffu, in_range);   // the lanes that take part in the solver's warp votes
   if (in_range) {
@@ -143,6 +144,17 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
     }
 #pragma unroll
     for (int v = 0; v < NPRIM; ++v) G.P[v][c] = P[v];
+    if (STAGE == 3 && G.wave_mode == WAVE_MHD_INSIDE) {
+      // a7 fused into the final recovery (f1): with state-dependent wave speeds the CFL reduction is a per-step one,
+      // and the new primitives are in registers here
+      Met m;
+      load_met_cell(G, c, m);
+      const bool mhd = P[RHO] > G.wave_rho_switch;
+      double Pq[NPRIM];
+#pragma unroll
+      for (int v = 0; v < NPRIM; ++v) Pq[v] = (mhd && (v <= VZ || (v >= BX && v <= BZ))) ? P[v] : 0.0;
+      cfl = cell_cfl_speed(m, G.Gamma, Pq, mhd, G.inv_dx[0], G.inv_dx[1], G.inv_dx[2], G.n[0] > 1, G.n[1] > 1, G.n[2] > 1);
+    }
     double sgE[3];
     const double iada = (STAGE == 3) ? 0.0 : rcp_fast(adt * alpha);
 #pragma unroll
@@ -175,6 +187,11 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       }
       stage_precombine<(STAGE == 4) ? 1 : STAGE>(G, c, dt, S, sgE, un, us, x1);
     }
+  }
+  if (STAGE == 3 && G.wave_mode == WAVE_MHD_INSIDE) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cfl = fmax(cfl, __shfl_xor_sync(0xffffffffu, cfl, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(G.maxspeed_word, (unsigned long long)__double_as_longlong(cfl));
   }
   // stats: warp reduce, one atomic per warp
   int fl = failed, fo = floored, mx = evmax;

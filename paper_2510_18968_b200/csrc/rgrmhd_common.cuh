@@ -50,6 +50,7 @@ struct GridView {
   double* X1[3];         // calE^(1) (needed again by the final combine, Eq. 37)
   double* dU[NCONS];     // w dt (-div F) of the last flux launch (w = 1 stage 1, 1/2 stage 2); the next recovery adds it
   double* src[NSRC];     // static source coefficients (metric derivatives, G^i, tr K; rgrmhd_sources.cuh)
+  unsigned long long* maxspeed_word;    // bit pattern of the running max of the CFL reduction (a7)
   const unsigned long long* src_mask;   // device word: bit q set <=> src[q] (q < NSRC) / K_ij[q - NSRC] is not identically 0
 };
 
@@ -480,6 +481,30 @@ __device__ __forceinline__ void mhd_speeds_nat(const Met& m, double Gamma, const
   lower(m, vU, vD); lower(m, BU, BD);
   mhd_speeds(m.alpha, m.b[K], m.gi[sym(K, K)], Gamma, Gamma / (Gamma - 1.0), P[RHO], P[PRS], dot3(vU, vD), dot3(BU, BD),
              dot3(BU, vD), vU[K], lm, lp);
+}
+
+// a7, one cell: max over the active directions of the CFL speed / dx -- Eq. 30, (alpha sqrt(gamma^kk) + |beta^k|)/dx^k,
+// or with wave mode MHD_INSIDE (reading R16) the cell's own max(|lambda-|, |lambda+|)/dx^k where rho > wave_rho_switch.
+// NOT inlined on purpose: the stand-alone reduction (k_max_speed) and the one fused into the final recovery call the
+// same compiled function, so the two give the same bits.
+static __device__ __noinline__ double cell_cfl_speed(const Met& m, double Gamma, const double P[NPRIM], bool mhd, double idx0,
+                                              double idx1, double idx2, bool a0, bool a1, bool a2) {
+  double s0, s1, s2;
+  if (mhd) {
+    double lm, lp;
+    mhd_speeds_nat<0>(m, Gamma, P, lm, lp); s0 = fmax(fabs(lm), fabs(lp));
+    mhd_speeds_nat<1>(m, Gamma, P, lm, lp); s1 = fmax(fabs(lm), fabs(lp));
+    mhd_speeds_nat<2>(m, Gamma, P, lm, lp); s2 = fmax(fabs(lm), fabs(lp));
+  } else {
+    s0 = m.alpha * sqrt(m.gi[0]) + fabs(m.b[0]);
+    s1 = m.alpha * sqrt(m.gi[3]) + fabs(m.b[1]);
+    s2 = m.alpha * sqrt(m.gi[5]) + fabs(m.b[2]);
+  }
+  double mx = 0.0;
+  if (a0) mx = fmax(mx, s0 * idx0);
+  if (a1) mx = fmax(mx, s1 * idx1);
+  if (a2) mx = fmax(mx, s2 * idx2);
+  return mx;
 }
 
 // a3 (second half). HLLE combination (Eq. 30; reading R6; wave speeds: reading R16)

@@ -254,22 +254,11 @@ k_max_speed(const __grid_constant__ GridView G, unsigned long long* __restrict__
     Met m;
     const long long c = cell_index(G, i, j, k);
     load_met_cell(G, c, m);
-    if (mhd_mode && G.P[RHO][c] > G.wave_rho_switch) {   // A9: the cell's own ideal-GRMHD speeds (reading R16)
-      double P[NPRIM];
+    const bool mhd = mhd_mode && G.P[RHO][c] > G.wave_rho_switch;   // A9: the cell's own ideal-GRMHD speeds (reading R16)
+    double P[NPRIM];
 #pragma unroll
-      for (int v = 0; v < NPRIM; ++v) P[v] = (v <= VZ || (v >= BX && v <= BZ)) ? G.P[v][c] : 0.0;
-      double lm[3], lp[3];
-      mhd_speeds_nat<0>(m, G.Gamma, P, lm[0], lp[0]);
-      mhd_speeds_nat<1>(m, G.Gamma, P, lm[1], lp[1]);
-      mhd_speeds_nat<2>(m, G.Gamma, P, lm[2], lp[2]);
-#pragma unroll
-      for (int d = 0; d < 3; ++d)
-        if (G.n[d] > 1) mx = fmax(mx, fmax(fabs(lm[d]), fabs(lp[d])) * G.inv_dx[d]);
-    } else {
-#pragma unroll
-      for (int d = 0; d < 3; ++d)
-        if (G.n[d] > 1) mx = fmax(mx, (m.alpha * sqrt(m.gi[sym(d, d)]) + fabs(m.b[d])) * G.inv_dx[d]);
-    }
+    for (int v = 0; v < NPRIM; ++v) P[v] = (mhd && (v <= VZ || (v >= BX && v <= BZ))) ? G.P[v][c] : 0.0;
+    mx = fmax(mx, cell_cfl_speed(m, G.Gamma, P, mhd, G.inv_dx[0], G.inv_dx[1], G.inv_dx[2], G.n[0] > 1, G.n[1] > 1, G.n[2] > 1));
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));

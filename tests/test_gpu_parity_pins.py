@@ -277,8 +277,14 @@ def test_wave_speed_mode_mhd_inside(binding, variant):
             for _ in range(4):
                 g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
             _compare(g, o, n, 1 / 40, TOL20, "mhd speeds 5 steps")
-            ms_g, ms_o = g.max_speed(), o.max_speed()                # pending final recovery is flushed first
+            g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)   # leaves the final recovery pending
+            l0 = g.launch_count()
+            ms_g, ms_o = g.max_speed(), o.max_speed()                # the pending final recovery is flushed first ...
+            assert g.launch_count() - l0 == 1                        # ... and reduces the CFL speed itself: one launch
             assert abs(ms_g - ms_o) <= 1e-12 * ms_o
+            assert g.max_speed() == ms_g and g.launch_count() - l0 == 1          # still valid: no launch at all
+            g.set_prims(g.get_prims())                               # same state, fused value forgotten:
+            assert g.max_speed() == ms_g                             # the stand-alone kernel gives the same bits
     w = wl.tov_like()
     i_surf = int(round((8.125 + 12.0) / w.dx[0]))
     nb, bc = (40, 12, 10), (wl.BC_OUTFLOW,) * 3
