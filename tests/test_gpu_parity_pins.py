@@ -446,3 +446,27 @@ def test_set_metric_twice_reallocates_the_static_source_fields(binding):
     ref.set_metric(flat); ref.set_prims(P)
     reused.step(0.005, wl.RECON_WENO5); ref.step(0.005, wl.RECON_WENO5)
     assert np.array_equal(ref.get_prims(), reused.get_prims())
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_superluminal_shift_upwinding(binding, variant):
+    """A shift beyond the light cone in every direction, of either sign: one of lambda+- is clipped to zero and HLLE is
+    pure upwinding (pinned for the oracle in tests/test_oracle_closed_forms.py); the CFL speed is alpha sqrt(g^kk) + |beta^k|."""
+    rng = np.random.default_rng(77)
+    n = (38, 21, 9)
+    shape = tuple(m + 6 for m in (n[2], n[1], n[0]))
+    m = np.zeros((16,) + shape); m[0] = 1.0; m[4] = m[7] = m[9] = 1.0
+    m[1], m[2], m[3] = 1.5, -1.4, 1.3
+    from test_oracle_scheme import _pad_periodic, _periodic_problem
+    _, P = _periodic_problem(40, rng, False)
+    sl = (slice(None), slice(0, n[2]), slice(0, n[1]), slice(0, n[0]))
+    P = _pad_periodic(np.ascontiguousarray(P[sl]))
+    par = dict(n=n, dx=(1 / 40,) * 3, bc=(0, 0, 0), gamma_eos=5 / 3, sigma0=30.0)
+    g, o = _both(binding, par, m, P, variant)
+    assert g.max_speed() == pytest.approx(2.5 * 40, rel=1e-15) and g.max_speed() == o.max_speed()
+    dt = 0.2 / (2.5 * 40)
+    g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+    _compare(g, o, n, 1 / 40, TOL1, "superluminal shift 1 step")
+    for _ in range(4):
+        g.step(dt, wl.RECON_WENO5); o.step(dt, wl.RECON_WENO5)
+    _compare(g, o, n, 1 / 40, TOL20, "superluminal shift 5 steps")

@@ -299,3 +299,40 @@ def test_face_fixups_pressure_density_fallback_and_velocity_limiter():
     o2.set_prims(_uniform_prims(o2.shape, 1.0, 1.0, (0.4999, 0, 0), (0, 0, 0), (0, 0, 0), 0, 0, 0))
     PL, PR, nf = o2.face_states(wl.RECON_MC, 0, 5)
     assert nf == 0 and PL[2] == 0.4999
+
+
+# ----------------------------------------------------------------------------------------------
+# HLLE with a shift (Eq. 30, reading R6): clipping makes it pure upwinding once |beta| exceeds the light speed
+# ----------------------------------------------------------------------------------------------
+def superluminal_shift_problem(sign):
+    """1D block, flat gamma, alpha = 1, uniform shift beta^x = sign * 1.5 (coordinates sweeping past the fluid faster
+    than light): lambda+ = max(0, 1 - beta) and lambda- = min(0, -1 - beta), so one of them is clipped to zero and the
+    HLLE flux is exactly the flux of the upwind state.  Piecewise-constant data, minmod (face states = cell values)."""
+    n = (16, 1, 1)
+    shape = (1, 1, 22)
+    m = _flat_metric(shape)
+    m[1] = sign * 1.5
+    rng = np.random.default_rng(12)
+    P = np.zeros((14,) + shape)
+    for c0, c1 in ((0, 9), (9, 15), (15, 22)):                   # three constant states
+        P[0, 0, 0, c0:c1] = rng.uniform(0.5, 1.5); P[1, 0, 0, c0:c1] = rng.uniform(0.5, 1.5)
+        for f in range(2, 14):
+            P[f, 0, 0, c0:c1] = rng.uniform(-0.3, 0.3)
+    return n, m, P
+
+
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_hlle_is_pure_upwinding_beyond_the_light_cone(sign):
+    n, m, P = superluminal_shift_problem(sign)
+    Gam, dx = 5 / 3, 0.1
+    o = oracle.Oracle(dict(n=n, dx=(dx, dx, dx), bc=(1, 1, 1), gamma_eos=Gam, sigma0=0.0, kappa=0.0))
+    o.set_metric(m); o.set_prims(P)
+    F = interior(o.rhs(wl.RECON_MINMOD), n)[:, 0, 0, :]
+    S = interior(o.sources(), n)[:, 0, 0, :]
+    beta = np.array([sign * 1.5, 0, 0])
+    flux = lambda c: oracle.state_flux_point(P[:, 0, 0, c], 0, Gam, 1.0, beta, None, 1, 0.0, 0.0)[1]
+    for i in range(16):
+        c = i + 3
+        # beta > c: both face fluxes come from the cell on the right of each face; beta < -c: from the left
+        exp = -(flux(c + 1) - flux(c)) / dx if sign > 0 else -(flux(c) - flux(c - 1)) / dx
+        assert np.allclose(F[:, i] - S[:, i], exp, rtol=1e-13, atol=1e-13), (sign, i)
