@@ -41,8 +41,9 @@ __device__ __forceinline__ void finish_face_met(const FaceRaw& w, FaceMet& m) {
   const double c01 = m.g[2] * m.g[4] - m.g[1] * m.g[5];
   const double c02 = m.g[1] * m.g[4] - m.g[2] * m.g[3];
   const double det = m.g[0] * c00 + m.g[1] * c01 + m.g[2] * c02;
-  const double idet = rcp_fast(det);
-  m.sg = sqrt_fast(det);
+  double rs;
+  sqrt_rsqrt_fast(det, m.sg, rs);
+  const double idet = rs * rs;
   m.gi0[0] = c00 * idet; m.gi0[1] = c01 * idet; m.gi0[2] = c02 * idet;
 }
 __device__ __forceinline__ void load_face_met(const PencilTabs& T, int K, long long cl, long long cr, FaceMet& m) {
@@ -117,8 +118,7 @@ __device__ __forceinline__ void half_flux(const FaceMet& m, double gog1, const d
   Gf[CQ] = U[CQ] * v[0] + Jc;
 #pragma unroll
   for (int c = 0; c < NCONS; ++c) {
-    const double t = wa * Gf[c] + wu * U[c];
-    Fh[c] = FIRST ? t : Fh[c] + t;
+    Fh[c] = FIRST ? fma(wa, Gf[c], wu * U[c]) : fma(wa, Gf[c], fma(wu, U[c], Fh[c]));
   }
 }
 
