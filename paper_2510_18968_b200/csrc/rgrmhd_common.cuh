@@ -410,6 +410,37 @@ __device__ __forceinline__ void recon_cells(double eps_w, const double (&u)[N][5
   }
 }
 
+// Upper-face value only (the halo cells of a tile need one face): the same expressions as the upper face of
+// weno5_pair, so the result is bit-identical; the lower-face value of a cell is this function of the mirrored stencil
+// (u4 .. u0), also bit for bit (the differences change sign and order, the indicators swap, every product keeps its
+// magnitude).
+template <int RECON>
+__device__ __forceinline__ double recon_hi(double eps_w, const double (&u)[5]) {
+  if (RECON == RECON_WENO5) {
+    const double D0 = u[1] - u[0], D1 = u[2] - u[1], D2 = u[3] - u[2], D3 = u[4] - u[3];
+    const double d0 = D1 - D0, e0 = fma(3.0, D1, -D0);
+    const double d1 = D2 - D1, e1 = D1 + D2;
+    const double d2 = D3 - D2, e2 = fma(-3.0, D2, D3);
+    const double e4 = 4.0 * eps_w;
+    const double b0 = fma((13.0 / 3.0) * d0, d0, fma(e0, e0, e4));
+    const double b1 = fma((13.0 / 3.0) * d1, d1, fma(e1, e1, e4));
+    const double b2 = fma((13.0 / 3.0) * d2, d2, fma(e2, e2, e4));
+    const double p12 = b1 * b2, p02 = b0 * b2, p01 = b0 * b1;
+    const double s12 = p12 * p12, s02 = p02 * p02, s01 = p01 * p01;
+    const double hA = fma(0.1 * 5.0 / 6.0, D1, (-0.1 * 2.0 / 6.0) * D0);
+    const double hB = fma(0.6 * 2.0 / 6.0, D2, (0.6 / 6.0) * D1);
+    const double hC = fma(0.3 * 4.0 / 6.0, D2, (-0.3 / 6.0) * D3);
+    const double hn = fma(s12, hA, fma(s02, hB, s01 * hC));
+    const double mid = 0.6 * s02;
+    const double hd = fma(0.1, s12, fma(0.3, s01, mid));
+    return fma(hn, rcp_fast(hd), u[2]);
+  } else {
+    const double a = u[2] - u[1], b = u[3] - u[2];
+    const double slope = (RECON == RECON_MINMOD) ? minmod2(a, b) : minmod3(2.0 * a, 2.0 * b, 0.5 * (a + b));
+    return u[2] + 0.5 * slope;
+  }
+}
+
 template <int RECON>
 __device__ __forceinline__ void recon_cell(double eps_w, double um2, double um1, double u0, double up1, double up2,
                                            double& lo, double& hi) {

@@ -254,16 +254,17 @@ k_flux_tma(const __grid_constant__ GridView G, const __grid_constant__ PencilTab
             __syncwarp();
             if (lane == 0) mbar_arrive(&S.empty[st]);
             if (mine) {
-              double l1[1], h1[1];
-              recon_cells<RECON, 1>(G.weno_eps, u, l1, h1);
-              double l = l1[0], h = h1[0];
-              if (vr < 2) {   // reading R4: unphysical face values fall back to the cell value
-                if (!(l > 0.0)) l = u[0][2];
-                if (!(h > 0.0)) h = u[0][2];
+              // one face per halo cell: the upper face of a cell below the tile, the lower face of a cell above it =
+              // the upper face of its mirrored stencil (bit-identical to the two-sided reconstruction, see recon_hi)
+              if (hup) {
+                double t = u[0][0]; u[0][0] = u[0][4]; u[0][4] = t;
+                t = u[0][1]; u[0][1] = u[0][3]; u[0][3] = t;
               }
+              double f = recon_hi<RECON>(G.weno_eps, u[0]);
+              if (vr < 2 && !(f > 0.0)) f = u[0][2];   // reading R4: unphysical face values fall back to the cell value
               if (hvalid) {
-                if (hup) S.exlo[vr][hr] = l;
-                else S.ex[vr][(K == 0) ? hr * EXW : hr] = h;
+                if (hup) S.exlo[vr][hr] = f;
+                else S.ex[vr][(K == 0) ? hr * EXW : hr] = f;
               }
             }
           }
