@@ -46,7 +46,8 @@ enum rgrmhd_status {
                             any call but set_prims/destroy after a launch inside rgrmhd_step failed
                             (the state is half advanced: the handle refuses to hand it out)      */
   RGRMHD_E_CUDA    = -3, /* a CUDA call failed; rgrmhd_last_cuda_error() returns its string    */
-  RGRMHD_E_NOMEM   = -4  /* device allocation failed                                            */
+  RGRMHD_E_NOMEM   = -4, /* device allocation failed                                            */
+  RGRMHD_E_TOO_LARGE = -5 /* rgrmhd_max_speed_static only: more cells than its fixed scratch array allows */
 };
 
 /* boundary conditions ("Neumann": copy nearest interior cell; PAPER.md:359 periodic) */
@@ -183,6 +184,33 @@ int rgrmhd_flush(rgrmhd_t h);
  * in mode LIGHT the value depends on the metric only, so calls after the first one per set_metric return the cached
  * result of that reduction without a launch. */
 int rgrmhd_max_speed(rgrmhd_t h, double* host_out);
+
+/* The same reduction for callers that may not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): STATELESS -- no handle, rgrmhd_create allocates -- and with its scratch memory
+ * in a fixed __device__ array of the library (65,792 bytes per GPU that loads the library, held until exit).  Calls
+ * no cudaMalloc, cudaFree or allocating library routine; enqueues one 256-byte cudaMemsetAsync and one kernel on
+ * `stream` (a cudaStream_t; NULL = the legacy default stream) of `device` and returns without synchronising.
+ *   n, dx            HOST arrays: interior cells and spacings; ghost width 3 in every direction with n > 1 (the
+ *                    field layout at the top of this file)
+ *   metric_dev       HOST array of 10 DEVICE pointers: alpha, beta^x y z, gamma_xx xy xz yy yz zz (padded fields)
+ *   prims_dev        HOST array of 14 DEVICE pointers (padded fields; rho, p, v^i, B^i are read); used in mode
+ *                    RGRMHD_WAVE_MHD_INSIDE only, may be NULL in mode RGRMHD_WAVE_LIGHT
+ *   max_speed_dev    DEVICE pointer to one double: the result, written by the kernel (valid once the stream has
+ *                    reached that point; nothing is retained)
+ * Unlike the other entry points every field pointer must be a device pointer on `device`: nothing is copied.
+ * Limit: n[0]*n[1]*n[2] <= RGRMHD_STATIC_MAX_CELLS (= 256^3: one partial maximum per 2048 cells, 8192 slots);
+ * beyond it the call returns RGRMHD_E_TOO_LARGE and touches nothing.  Otherwise RGRMHD_E_INVALID (null pointer,
+ * n < 1, dx <= 0, unknown mode, Gamma <= 1 in mode MHD_INSIDE, device outside 0..63) or RGRMHD_E_CUDA.
+ * Every call on a GPU shares the ONE scratch array, which keeps the last call's contents (the call clears the part
+ * that has to start at zero): calls whose kernels can overlap on the GPU -- different streams, different host
+ * threads, two captured graphs run concurrently -- RACE; calls on one stream are ordered and safe.  The first call
+ * per device looks up the array's device address (cudaGetSymbolAddress; this may load the library's device code):
+ * make it once outside a capture.  Result: the same per-cell arithmetic as rgrmhd_max_speed and an exact maximum,
+ * so the two agree. */
+#define RGRMHD_STATIC_MAX_CELLS 16777216LL
+int rgrmhd_max_speed_static(const int n[3], const double dx[3], const double* const metric_dev[10],
+                            const double* const prims_dev[14], double gamma_eos, int wave_speed_mode,
+                            double wave_rho_switch, int device, void* stream, double* max_speed_dev);
 
 /* Current primitives (ghost zones filled by the boundary rule) / conserved variables
  * D,Sx,Sy,Sz,tau,calE(3),calB(3),Psi,Phi,calQ (interior valid; ghosts unspecified). */

@@ -24,7 +24,7 @@ NMETRIC = 16
 SYMBOLS = ["rgrmhd_params_default", "rgrmhd_create", "rgrmhd_destroy", "rgrmhd_set_stream", "rgrmhd_set_metric",
            "rgrmhd_set_sigma", "rgrmhd_set_prims", "rgrmhd_step", "rgrmhd_max_speed", "rgrmhd_get_prims",
            "rgrmhd_get_cons", "rgrmhd_get_stats", "rgrmhd_reset_stats", "rgrmhd_set_rhs_variant", "rgrmhd_get_rhs_variant", "rgrmhd_step_begin", "rgrmhd_step_continue", "rgrmhd_halo_doubles",
-           "rgrmhd_halo_pack", "rgrmhd_halo_unpack",
+           "rgrmhd_halo_pack", "rgrmhd_halo_unpack", "rgrmhd_max_speed_static",
            "rgrmhd_launch_count", "rgrmhd_flush", "rgrmhd_set_timing", "rgrmhd_get_timing", "rgrmhd_measure_fp64_peak",
            "rgrmhd_strerror", "rgrmhd_last_cuda_error"]
 
@@ -137,6 +137,29 @@ def _ptr(a) -> int:
 def _table(arrs: Sequence) -> "C.Array":
     T = C.c_void_p * len(arrs)
     return T(*[_ptr(a) for a in arrs])
+
+
+STATIC_MAX_CELLS = 16777216   # RGRMHD_STATIC_MAX_CELLS
+E_TOO_LARGE = -5              # RGRMHD_E_TOO_LARGE
+
+
+def max_speed_static(n, dx, metric, prims, gamma_eos: float, wave_speed_mode: int, wave_rho_switch: float, out,
+                     device: int = 0, stream: int = 0) -> None:
+    """rgrmhd_max_speed_static: the CFL reduction without a handle and without any allocation (scratch in a fixed
+    device array of the library).  ``metric``: the first 10 padded fields of the metric stack (alpha, beta, gamma) as
+    CUDA tensors; ``prims``: the 14 padded primitive fields as CUDA tensors, or None in mode LIGHT; ``out``: a CUDA
+    float64 tensor of one element, written asynchronously on ``stream``.  Argument marshalling only."""
+    L = load()
+    ni = (C.c_int * 3)(*[int(v) for v in n])
+    dxi = (C.c_double * 3)(*[float(v) for v in dx])
+    for a in list(metric[:10]) + (list(prims) if prims is not None else []) + [out]:
+        assert getattr(a, "is_cuda", False), "rgrmhd_max_speed_static takes device pointers only"
+    rc = L.rgrmhd_max_speed_static(ni, dxi, _table([metric[i] for i in range(10)]),
+                                   _table([prims[i] for i in range(NPRIM)]) if prims is not None else None,
+                                   C.c_double(gamma_eos), int(wave_speed_mode), C.c_double(wave_rho_switch), int(device),
+                                   C.c_void_p(stream), C.c_void_p(_ptr(out)))
+    if rc != 0:
+        raise RgrmhdError("rgrmhd_max_speed_static", rc)
 
 
 class Rgrmhd:

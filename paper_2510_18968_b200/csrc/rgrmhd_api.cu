@@ -813,6 +813,7 @@ const char* rgrmhd_strerror(int code) {
     case RGRMHD_E_STATE: return "call out of order (metric / primitives / sigma not set, wrong sigma model, or a failed step left the state unusable until set_prims)";
     case RGRMHD_E_CUDA: return "CUDA error (see rgrmhd_last_cuda_error)";
     case RGRMHD_E_NOMEM: return "device allocation failed";
+    case RGRMHD_E_TOO_LARGE: return "more cells than the fixed scratch array of rgrmhd_max_speed_static allows (RGRMHD_STATIC_MAX_CELLS)";
   }
   return "unknown status";
 }
