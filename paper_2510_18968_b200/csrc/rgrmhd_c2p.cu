@@ -47,6 +47,10 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
 #pragma unroll
     for (int q = 0; q < 6; ++q) g6[q] = __ldg(G.met[MGXX + q] + c);
     const double alpha = __ldg(G.met[MALP] + c);
+    // loads that depend on nothing but the cell index go out with the first batch: left inside sigma_of / behind the
+    // first solve they each cost a DRAM round trip of their own (measured: -2 % of this kernel on config 4)
+    const double sig_arr = (STAGE != 3 && G.sigma_model == SIGMA_ARRAY) ? __ldg(G.sigma + c) : 0.0;
+    const unsigned long long nz = (STAGE != 3) ? __ldg(G.src_mask) : 0ull;
     Triad t;
     triad_make(g6, t);
     const double sg = t.l11 * t.l22 * t.l33;
@@ -88,7 +92,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
         for (int q = 0; q < 3; ++q) { U[CSX + q] = Unew[CSX + q]; Ust[CSX + q][c] = U[CSX + q]; }
       }
     }
-    const double sigma = (STAGE == 3) ? 0.0 : sigma_of(G, U[CD] * isg, c);
+    const double sigma = (STAGE == 3) ? 0.0 : (G.sigma_model == SIGMA_ARRAY) ? sig_arr : sigma_of(G, U[CD] * isg, c);
     // The point-wise right-hand side after the solve reads ~57 more fields of this cell.  Start those loads
     // now as asynchronous copies into a thread-private shared-memory column: no registers are held and
     // the solve below hides their DRAM latency.
@@ -97,7 +101,6 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
     constexpr int NTH = C2P_TX * C2P_TY;
     if (STAGE != 3) {
       // fields that are identically zero on this grid (zero shift, K_ij = 0, diagonal metric, ...) are not read
-      const unsigned long long nz = __ldg(G.src_mask);
 #pragma unroll
       for (int q = 0; q < NSRC; ++q) {
         if ((nz >> q) & 1ull) cp_async8(pf + (PF_SRC + q) * NTH, G.src[q] + c);
