@@ -40,7 +40,6 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
   int evals = 0, evmax = 0, failed = 0, floored = 0;
   double cfl = 0.0;
   const bool in_range = i < G.n[0] && j < G.n[1];
-  const unsigned lanes = __ballot_sync(0xffffffffu, in_range);   // the lanes that take part in the solver's warp votes
   if (in_range) {
     const long long c = cell_index(G, i, j, k);
     double g6[6];
@@ -73,7 +72,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
     const double isg = rcp_fast(sg);
     if (STAGE == 4) {
       // deferred final recovery of the previous step (a = 0): its primitives are the guess of the stage-1 solve
-      C2POut r0 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, 0.0, 0.0, G.tol, G.maxit, lanes, P);
+      C2POut r0 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, 0.0, 0.0, G.tol, G.maxit, P);
       evals = evmax = r0.evals; failed = r0.failed;
       if (G.rho_floor > 0.0 && (r0.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {
         // reading R9: atmosphere reset with write-back, as in STAGE 3
@@ -124,7 +123,7 @@ k_c2p(const __grid_constant__ GridView G, double dt, StatsDev* __restrict__ stat
       }
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
-    C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, lanes, P);
+    C2POut r2 = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, P);
     evals += r2.evals; failed += r2.failed;
     evmax = max(evmax, r2.evals);
     if (G.rho_floor > 0.0 && (r2.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {

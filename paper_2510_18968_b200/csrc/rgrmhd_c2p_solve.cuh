@@ -12,7 +12,8 @@
 // (Cholesky factor, gamma = L L^T): every dot and cross product in the loop is Euclidean and the
 // metric is touched only before and after.  The solver is ONE loop whose body holds exactly one
 // residual evaluation, so lanes in different inner/outer phases still execute the expensive part
-// convergently; the loop ends for a warp when every lane is done (warp vote).
+// convergently; a lane leaves the loop when it is done and waits for the rest of its warp at the loop's exit (an
+// explicit warp vote per trip, the round-1 version, measured 3 % slower for the whole kernel).
 #pragma once
 #include "rgrmhd_sources.cuh"
 
@@ -70,7 +71,7 @@ __device__ __forceinline__ void implicit_E_closed(const double v[3], double W, d
 // P holds the guess (rho, p, v^i) on entry and all 14 primitives on return.  sg = sqrt(gamma).
 __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double alpha, double Gamma, double gog1,
                                             double gm1og, const double U[NCONS], double adt, double sigma, double tol,
-                                            int maxit, unsigned lanes, double P[NPRIM]) {
+                                            int maxit, double P[NPRIM]) {
   const double Dh = U[CD] * isg, tauh = U[CTAU] * isg;
   double Sh[3], Es[3], B[3], EsxB[3];
   triad_from_cov(t, U[CSX] * isg, U[CSY] * isg, U[CSZ] * isg, Sh);
@@ -98,7 +99,7 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
   double W = Wg;
   double kE = dot3(vg, Es) * W * rcp_fast(W + s0);          // (v.E*)/(1 + s/W^2), s = s0 W
   // no physical bracket: a failure; keep the guess, E from the guess v (the tail below does exactly that for a lane
-  // without a valid state).  Such a lane must NOT leave early: the loop's warp vote names every lane that entered.
+  // without a valid state): such a lane never enters the loop.
   const bool no_bracket = !(Dh > 0.0) || !(Zhi > Zlo);
   double Z = (P[RHO] + gog1 * P[PRS]) * W * W;
   bool converged = false, state_ok = false;
@@ -116,8 +117,8 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
   int outer = 0;
   bool need_setup = true, done = no_bracket;
   // ONE loop, one residual evaluation per trip.
-  while (true) {
-    if (!done) {
+  while (!done) {
+    {
       if (need_setup) {
         // ---- outer pass set-up: freeze (s, kE), decompose N along/across B ---------------------
         s = s0 * W; i1s = rcp_fast(1.0 + s); r = s * i1s;
@@ -210,7 +211,6 @@ __device__ __forceinline__ C2POut c2p_solve(const Triad& t, double isg, double a
         }
       }
     }
-    if (__all_sync(lanes, done)) break;                     // warp-vote exit over the lanes that entered the solve
   }
   res.failed = converged ? 0 : 1;
   double EU[3];

@@ -42,7 +42,6 @@ k_stage_gen(const __grid_constant__ GridView G, const __grid_constant__ StageGen
   const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
   int evals = 0, failed = 0, floored = 0;
   const bool in_range = i < G.n[0];
-  const unsigned lanes = __ballot_sync(0xffffffffu, in_range);
   if (in_range) {
     const long long c = cell_index(G, i, j, k);
     const int me = FINAL ? 4 : W.stage;
@@ -64,7 +63,7 @@ k_stage_gen(const __grid_constant__ GridView G, const __grid_constant__ StageGen
     for (int v = 0; v < 5; ++v) P[v] = G.P[v][c];
     const double adt = FINAL ? 0.0 : W.aii * dt;
     const double sigma = FINAL ? 0.0 : sigma_of(G, U[CD] * isg, c);
-    C2POut r = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, lanes, P);
+    C2POut r = c2p_solve(t, isg, alpha, G.Gamma, G.gog1, G.gm1og, U, adt, sigma, G.tol, G.maxit, P);
     evals = r.evals; failed = r.failed;
     if (G.rho_floor > 0.0 && (r.failed || !(P[RHO] > G.rho_floor * (1.0 + 1e-3)))) {   // reading R9
       floored = 1;
